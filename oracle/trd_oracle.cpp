@@ -1,0 +1,586 @@
+// trd_oracle.cpp -- ORACLE.  TEST INFRASTRUCTURE, NOT THE PRODUCT.
+//
+// A plain, slow, double-precision CPU implementation of the online TRD tracking step of
+// arXiv 2003.03174 (section 3, Fig. 2 L40): ITS-TPC seed tracks are
+// propagated through the six TRD layers, the tracklets inside a search road are scored by
+// chi2, the best N hypotheses are kept per layer and updated with a Kalman filter.
+//
+// Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs
+// may build, load or call this file.  It shares no code, header, table or helper with the
+// CUDA path under paper_2003_03174_b200/csrc/ and includes nothing from include/.
+//
+// The method is a heuristic beam search, so this file is the algorithm written out step by
+// step; full 5x5 matrices, std::sort, std::lower_bound, no blocking
+// or fusion.  The paper prints no equation for the track model, road, chi2, gain or ranking;
+// every reading taken is listed in DESIGN.md ("Readings") and referenced as [R#] below.
+//
+// Pins (tests/test_oracle_*.py, all -m "not gpu"): closed-form straight line at Bz = 0,
+// analytic circle crossing, composition and inverse of propagation, finite-difference
+// Jacobians, information-form Kalman update via numpy.linalg, batch least squares, exact
+// recovery on noise-free input, unit pulls and <chi2> = ndf on smeared input, index ==
+// brute force, beam search == exhaustive chain enumeration, nHyp = 1 == greedy matcher.
+// No function here is "parity unpinned".
+//
+// Conventions [R1]: sector frame s rotated by (s + 1/2) * 20 deg about z; state at local x is
+// p = (y, z, sin(phi), tan(lambda), q/pT [c/GeV]); cos(phi) > 0 implied; curvature
+// kappa = b * q/pT with b = -0.00299792458 * Bz[T] per cm; cm, Tesla, GeV/c.  Covariance is
+// the symmetric 5x5 matrix; the 15-element interface order is the lower triangle row by row
+// (yy, zy, zz, sy, sz, ss, ty, tz, ts, tt, cy, cz, cs, ct, cc).
+
+#include <algorithm>
+#include <chrono>
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <limits>
+#include <vector>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+namespace {
+
+constexpr int kMaxLayers = 6;
+constexpr double kLoose = 1e-2;   // slack used only to decide which margins are worth recording
+
+struct Config {
+    int32_t n_sectors, n_stacks, n_layers, n_hyp;
+    double layer_x[kMaxLayers];
+    double z_max, pad_length, bz_tesla;
+    double sigma_y, sigma_z, sigma_dydx;
+    double n_sigma_road, n_sigma_angle;
+    double chi2_cut, chi2_penalty, max_snp;
+};
+
+struct Hyp {
+    double p[5];
+    double C[5][5];
+    double x;
+    int sector;
+    double score;      // sum of chi2 increments + penalty * skipped layers   [R5]
+    double chi2;       // sum of chi2 increments only
+    int idx[kMaxLayers];
+    int n_matched;
+    bool alive;
+};
+
+struct Tracklet {
+    double y, z, dydx;
+    int index;         // position in the caller's arrays
+};
+
+struct Counters {
+    int64_t n_prop = 0, n_rot = 0, n_road = 0, n_cand = 0, n_upd = 0, n_scanned = 0;
+};
+
+inline double curvature_factor(const Config& cfg) { return -0.00299792458 * cfg.bz_tesla; }
+
+inline void note(double* margin, double value, double threshold) {
+    // relative distance of a quantity from the threshold it is compared with
+    if (!margin) return;
+    double m = std::fabs(value - threshold) / std::fabs(threshold);
+    if (m < *margin) *margin = m;
+}
+
+// (asin(w) - w) / w^2, with its series near 0
+inline double q_of(double w) {
+    if (std::fabs(w) < 1e-2) {
+        double w2 = w * w;
+        return w * (1.0 / 6.0 + w2 * (3.0 / 40.0 + w2 * (15.0 / 336.0 + w2 * (105.0 / 3456.0))));
+    }
+    return (std::asin(w) - w) / (w * w);
+}
+
+// ---- propagation x0 -> x1 inside one sector frame, uniform Bz, no material ---------------
+// PAPER.md:52 ("extrapolated to the first TRD layer"); formulas SURVEY.md 8(c).3.
+// Returns false (state untouched) if |sin(phi)| would reach max_snp [R14].  F, if given,
+// receives the 5x5 Jacobian d(y',z',s',t',c')/d(y,z,s,t,c).
+bool propagate_state(const Config& cfg, const double p[5], double x0, double x1, double out[5],
+                     double F[5][5], double* margin) {
+    const double b = curvature_factor(cfg);
+    const double dx = x1 - x0;
+    const double y = p[0], z = p[1], s = p[2], t = p[3], c = p[4];
+    const double kappa = b * c;
+    const double u = kappa * dx;
+    const double f1 = s, f2 = s + u;
+    note(margin, std::fabs(f2), cfg.max_snp);
+    if (std::fabs(f1) >= 1.0 || std::fabs(f2) >= cfg.max_snp) return false;
+    const double r1 = std::sqrt(1.0 - f1 * f1), r2 = std::sqrt(1.0 - f2 * f2);
+    const double cosd = r1 * r2 + f1 * f2;               // cos of the turning angle
+    const double g = (1.0 + cosd) / (r1 + r2);
+    const double w = u * g;                              // sin of the turning angle
+    const double asw = (std::fabs(w) < 1e-8) ? 1.0 : std::asin(w) / w;
+    const double ell = dx * g * asw;                     // xy path length
+    out[0] = y + dx * (f1 + f2) / (r1 + r2);
+    out[1] = z + t * ell;
+    out[2] = f2;
+    out[3] = t;
+    out[4] = c;
+    if (F) {
+        for (int i = 0; i < 5; ++i)
+            for (int j = 0; j < 5; ++j) F[i][j] = (i == j) ? 1.0 : 0.0;
+        const double h = f2 * g / (r2 * (r1 + r2)) - g * g * q_of(w);
+        F[0][2] = dx * g / (r1 * r2);
+        F[0][4] = b * dx * dx * g / (r2 * (r1 + r2));
+        F[1][2] = t * dx * (f1 + f2) / (r1 * r2 * (r1 + r2));
+        F[1][3] = ell;
+        F[1][4] = b * t * dx * dx * h;
+        F[2][4] = b * dx;
+    }
+    return true;
+}
+
+void similarity(const double A[5][5], double C[5][5]) {   // C <- A C A^T, full matrices
+    double T[5][5], R[5][5];
+    for (int i = 0; i < 5; ++i)
+        for (int j = 0; j < 5; ++j) {
+            double acc = 0.0;
+            for (int k = 0; k < 5; ++k) acc += A[i][k] * C[k][j];
+            T[i][j] = acc;
+        }
+    for (int i = 0; i < 5; ++i)
+        for (int j = 0; j < 5; ++j) {
+            double acc = 0.0;
+            for (int k = 0; k < 5; ++k) acc += T[i][k] * A[j][k];
+            R[i][j] = acc;
+        }
+    for (int i = 0; i < 5; ++i)
+        for (int j = 0; j < 5; ++j) C[i][j] = 0.5 * (R[i][j] + R[j][i]);
+}
+
+bool propagate(const Config& cfg, Hyp& h, double x1, double* margin, Counters* cnt) {
+    double out[5], F[5][5];
+    if (cnt) cnt->n_prop++;
+    if (!propagate_state(cfg, h.p, h.x, x1, out, F, margin)) return false;
+    std::memcpy(h.p, out, sizeof out);
+    similarity(F, h.C);
+    h.x = x1;
+    return true;
+}
+
+// ---- rotation of the frame by beta about z at the current point ------
+// Same physical point and direction, new frame; the Jacobian brings a perturbed track back
+// to the plane x' = const of the new frame.
+bool rotate_state(const Config& cfg, const double p[5], double x, double beta, double out[5],
+                  double* x_out, double J[5][5], double* margin) {
+    const double cb = std::cos(beta), sb = std::sin(beta);
+    const double y = p[0], s = p[2], t = p[3];
+    if (std::fabs(s) >= 1.0) return false;
+    const double r = std::sqrt(1.0 - s * s);
+    const double s2 = s * cb - r * sb;
+    const double c2 = r * cb + s * sb;                    // cos(phi) in the new frame
+    note(margin, std::fabs(s2), cfg.max_snp);
+    if (std::fabs(s2) >= cfg.max_snp || c2 <= 0.0) return false;
+    const double r2 = std::sqrt(1.0 - s2 * s2);
+    *x_out = x * cb + y * sb;
+    out[0] = -x * sb + y * cb;
+    out[1] = p[1];
+    out[2] = s2;
+    out[3] = p[3];
+    out[4] = p[4];
+    if (J) {
+        const double kappa = curvature_factor(cfg) * p[4];
+        for (int i = 0; i < 5; ++i)
+            for (int j = 0; j < 5; ++j) J[i][j] = (i == j) ? 1.0 : 0.0;
+        J[0][0] = r / r2;
+        J[1][0] = -t * sb / r2;
+        J[2][0] = -kappa * sb;
+        J[2][2] = r2 / r;
+    }
+    return true;
+}
+
+bool rotate(const Config& cfg, Hyp& h, double beta, double* margin, Counters* cnt) {
+    double out[5], J[5][5], xn;
+    if (cnt) cnt->n_rot++;
+    if (!rotate_state(cfg, h.p, h.x, beta, out, &xn, J, margin)) return false;
+    std::memcpy(h.p, out, sizeof out);
+    similarity(J, h.C);
+    h.x = xn;
+    return true;
+}
+
+// propagate to the layer plane x = X; change sector while |y| is beyond the sector edge
+// X tan(10 deg), at most twice [R14].  On failure the hypothesis is left untouched.
+bool propagate_to_layer(const Config& cfg, Hyp& h, double X, double* margin, Counters* cnt) {
+    Hyp w = h;
+    const double half = M_PI / cfg.n_sectors;
+    const double edge = X * std::tan(half);
+    if (!propagate(cfg, w, X, margin, cnt)) return false;
+    for (int n_rot = 0;; ++n_rot) {
+        note(margin, std::fabs(w.p[0]), edge);
+        if (std::fabs(w.p[0]) <= edge) break;
+        if (n_rot == 2) return false;
+        const double beta = (w.p[0] > 0.0 ? 2.0 : -2.0) * half;
+        if (!rotate(cfg, w, beta, margin, cnt)) return false;
+        w.sector = (w.sector + (beta > 0.0 ? 1 : cfg.n_sectors - 1)) % cfg.n_sectors;
+        if (!propagate(cfg, w, X, margin, cnt)) return false;
+    }
+    h = w;
+    return true;
+}
+
+// ---- measurement model: m = (y, z), H = first two rows of I, R = diag(sy^2, sz^2) [R3,R10]
+struct Road {
+    double Sinv[2][2];
+    double road_y, road_z, tanphi;
+};
+
+Road make_road(const Config& cfg, const Hyp& h) {
+    Road rd;
+    const double S00 = h.C[0][0] + cfg.sigma_y * cfg.sigma_y;
+    const double S01 = h.C[1][0];
+    const double S11 = h.C[1][1] + cfg.sigma_z * cfg.sigma_z;
+    const double det = S00 * S11 - S01 * S01;
+    rd.Sinv[0][0] = S11 / det;
+    rd.Sinv[0][1] = rd.Sinv[1][0] = -S01 / det;
+    rd.Sinv[1][1] = S00 / det;
+    rd.road_y = cfg.n_sigma_road * std::sqrt(S00);                                   // [R2]
+    rd.road_z = cfg.n_sigma_road * std::sqrt(h.C[1][1]) + 0.5 * cfg.pad_length;      // [R2]
+    rd.tanphi = h.p[2] / std::sqrt(1.0 - h.p[2] * h.p[2]);
+    return rd;
+}
+
+inline double chi2_of(const Road& rd, double ry, double rz) {
+    return ry * (rd.Sinv[0][0] * ry + rd.Sinv[0][1] * rz) + rz * (rd.Sinv[1][0] * ry + rd.Sinv[1][1] * rz);
+}
+
+// Kalman update with the measurement (ym, zm), plain gain form
+double kalman_update(const Config& cfg, Hyp& h, double ym, double zm) {
+    const Road rd = make_road(cfg, h);
+    const double r[2] = {ym - h.p[0], zm - h.p[1]};
+    const double chi2inc = chi2_of(rd, r[0], r[1]);
+    double K[5][2];
+    for (int i = 0; i < 5; ++i)
+        for (int j = 0; j < 2; ++j) K[i][j] = h.C[i][0] * rd.Sinv[0][j] + h.C[i][1] * rd.Sinv[1][j];
+    for (int i = 0; i < 5; ++i) h.p[i] += K[i][0] * r[0] + K[i][1] * r[1];
+    double N[5][5];
+    for (int i = 0; i < 5; ++i)
+        for (int j = 0; j < 5; ++j) N[i][j] = h.C[i][j] - (K[i][0] * h.C[0][j] + K[i][1] * h.C[1][j]);
+    for (int i = 0; i < 5; ++i)
+        for (int j = 0; j < 5; ++j) h.C[i][j] = 0.5 * (N[i][j] + N[j][i]);
+    return chi2inc;
+}
+
+// ---- tracklet store: one list per (sector, layer), sorted by y --------------------------
+struct Store {
+    int n_sectors = 0, n_layers = 0;
+    std::vector<std::vector<Tracklet>> cell;   // [sector * n_layers + layer]
+    bool sorted = false;
+};
+
+void build_store(const Config& cfg, const float* y, const float* z, const float* dydx, const int32_t* chamber,
+                 int64_t n, bool sort_by_y, Store& st) {
+    st.n_sectors = cfg.n_sectors;
+    st.n_layers = cfg.n_layers;
+    st.cell.assign((size_t)cfg.n_sectors * cfg.n_layers, {});
+    const int per_sector = cfg.n_stacks * cfg.n_layers;
+    for (int64_t i = 0; i < n; ++i) {
+        const int ch = chamber[i];
+        if (ch < 0 || ch >= cfg.n_sectors * per_sector) continue;             // unusable tracklet
+        if (!std::isfinite(y[i]) || !std::isfinite(z[i])) continue;
+        const int sector = ch / per_sector, layer = ch % cfg.n_layers;        // stack id unused [R12]
+        st.cell[(size_t)sector * cfg.n_layers + layer].push_back({(double)y[i], (double)z[i], (double)dydx[i], (int)i});
+    }
+    if (sort_by_y)
+        for (auto& v : st.cell)
+            std::sort(v.begin(), v.end(), [](const Tracklet& a, const Tracklet& b) {
+                return a.y < b.y || (a.y == b.y && a.index < b.index);
+            });
+    st.sorted = sort_by_y;
+}
+
+struct Cand {
+    int index;
+    double y, z, chi2inc;
+};
+
+// all tracklets of the hypothesis' sector and layer inside the road, past the inclination
+// veto and the chi2 cut [R2,R3,R4,R8,R13]
+void find_candidates(const Config& cfg, const Store& st, const Hyp& h, int layer, const Road& rd,
+                     std::vector<Cand>& out, int* n_evals, double* margin, Counters* cnt) {
+    out.clear();
+    const std::vector<Tracklet>& v = st.cell[(size_t)h.sector * st.n_layers + layer];
+    size_t lo = 0, hi = v.size();
+    if (st.sorted) {
+        const double wide = rd.road_y * (1.0 + kLoose);
+        lo = std::lower_bound(v.begin(), v.end(), h.p[0] - wide,
+                              [](const Tracklet& a, double val) { return a.y < val; }) - v.begin();
+        hi = std::upper_bound(v.begin(), v.end(), h.p[0] + wide,
+                              [](double val, const Tracklet& a) { return val < a.y; }) - v.begin();
+    }
+    const double veto = cfg.n_sigma_angle * cfg.sigma_dydx;
+    for (size_t k = lo; k < hi; ++k) {
+        const Tracklet& tl = v[k];
+        if (cnt) cnt->n_scanned++;
+        const double ry = tl.y - h.p[0], rz = tl.z - h.p[1];
+        const double da = std::fabs(tl.dydx - rd.tanphi);
+        const bool in_y = std::fabs(ry) <= rd.road_y, in_z = std::fabs(rz) <= rd.road_z;
+        const bool pass = da <= veto;                                       // PAPER.md:60, 4 sigma [R8]
+        const bool loose_y = std::fabs(ry) <= rd.road_y * (1.0 + kLoose);
+        const bool loose_z = std::fabs(rz) <= rd.road_z * (1.0 + kLoose);
+        const bool loose_a = da <= veto * (1.0 + kLoose);
+        if (loose_z && loose_a) note(margin, std::fabs(ry), rd.road_y);
+        if (loose_y && loose_a) note(margin, std::fabs(rz), rd.road_z);
+        if (loose_y && loose_z) note(margin, da, veto);
+        const double c2 = chi2_of(rd, ry, rz);                              // y and z only
+        if (loose_y && loose_z && loose_a) note(margin, c2, cfg.chi2_cut);
+        if (!(in_y && in_z && pass)) continue;
+        if (n_evals) (*n_evals)++;                                          // one "candidate evaluation"
+        if (cnt) cnt->n_cand++;
+        if (c2 >= cfg.chi2_cut) continue;                                   // per-layer cut [R4]
+        out.push_back({tl.index, tl.y, tl.z, c2});
+    }
+}
+
+struct Child {
+    int parent;        // position of the parent in the current hypothesis list
+    int tracklet;      // caller's index, or INT_MAX for the skip-child (sorts after tracklets) [R6]
+    double y, z, score, chi2inc;
+};
+
+struct TrackResult {
+    Hyp best;
+    int n_evals;
+    double margin;
+};
+
+// one track through all layers; "only the best N_candidates
+// hypotheses are propagated", Fig. 2
+void match_track(const Config& cfg, const Store& st, const Hyp& seed, TrackResult& res, Counters* cnt) {
+    std::vector<Hyp> hyps(1, seed), next;
+    std::vector<Hyp> prop;
+    std::vector<Child> children;
+    std::vector<Cand> cands;
+    res.n_evals = 0;
+    res.margin = std::numeric_limits<double>::infinity();
+    double* mg = &res.margin;
+    for (int L = 0; L < cfg.n_layers; ++L) {
+        children.clear();
+        prop = hyps;                                        // propagated copies of the parents
+        for (int ih = 0; ih < (int)hyps.size(); ++ih) {
+            Hyp& h = prop[ih];
+            if (h.alive) h.alive = propagate_to_layer(cfg, h, cfg.layer_x[L], mg, cnt);
+            if (h.alive) {
+                const Road rd = make_road(cfg, h);
+                if (cnt) cnt->n_road++;
+                find_candidates(cfg, st, h, L, rd, cands, &res.n_evals, mg, cnt);
+                for (const Cand& c : cands)
+                    children.push_back({ih, c.index, c.y, c.z, h.score + c.chi2inc, c.chi2inc});
+            }
+            children.push_back({ih, std::numeric_limits<int>::max(), 0.0, 0.0, h.score + cfg.chi2_penalty, 0.0});
+        }
+        std::stable_sort(children.begin(), children.end(), [](const Child& a, const Child& b) {
+            if (a.score != b.score) return a.score < b.score;
+            if (a.parent != b.parent) return a.parent < b.parent;
+            return a.tracklet < b.tracklet;
+        });
+        const int keep = std::min<int>(cfg.n_hyp, (int)children.size());
+        // ranking margins: the keep boundary at every layer, the winner at the last layer
+        if ((int)children.size() > keep) {
+            const double a = children[keep - 1].score, b = children[keep].score;
+            const double m = (b - a) / std::max(std::fabs(b), 1e-300);
+            if (m < *mg) *mg = m;
+        }
+        if (L == cfg.n_layers - 1 && children.size() > 1) {
+            const double a = children[0].score, b = children[1].score;
+            const double m = (b - a) / std::max(std::fabs(b), 1e-300);
+            if (m < *mg) *mg = m;
+        }
+        next.clear();
+        for (int k = 0; k < keep; ++k) {
+            const Child& c = children[k];
+            Hyp h = prop[c.parent];
+            h.score = c.score;
+            if (c.tracklet != std::numeric_limits<int>::max()) {
+                const double chi2inc = kalman_update(cfg, h, c.y, c.z);
+                if (cnt) cnt->n_upd++;
+                h.chi2 += chi2inc;
+                h.idx[L] = c.tracklet;
+                h.n_matched++;
+                note(mg, std::fabs(h.p[2]), cfg.max_snp);
+                if (std::fabs(h.p[2]) >= cfg.max_snp) h.alive = false;     // kept, but only skips from now on
+            }
+            next.push_back(h);
+        }
+        hyps.swap(next);
+    }
+    res.best = hyps[0];
+}
+
+inline int tri(int i, int j) { return i * (i + 1) / 2 + j; }
+
+void load_hyp(Hyp& h, const double p[5], const double c15[15], double x, int sector) {
+    std::memset(&h, 0, sizeof h);
+    for (int i = 0; i < 5; ++i) h.p[i] = p[i];
+    for (int i = 0; i < 5; ++i)
+        for (int j = 0; j <= i; ++j) h.C[i][j] = h.C[j][i] = c15[tri(i, j)];
+    h.x = x;
+    h.sector = sector;
+    for (int l = 0; l < kMaxLayers; ++l) h.idx[l] = -1;
+    h.alive = true;
+}
+
+void store_cov(const Hyp& h, double c15[15]) {
+    for (int i = 0; i < 5; ++i)
+        for (int j = 0; j <= i; ++j) c15[tri(i, j)] = h.C[i][j];
+}
+
+}  // namespace
+
+// =========================================================================================
+// C entry points for the Python wrapper (oracle/oracle.py).  Own names, own struct layout.
+// =========================================================================================
+extern "C" {
+
+typedef Config orc_config;
+
+int orc_sizeof_config(void) { return (int)sizeof(Config); }
+
+// in-frame propagation of state + 15-element covariance; F25 (row-major 5x5) optional
+int orc_propagate(const orc_config* cfg, double p[5], double c15[15], double* x, double x_new, double* F25) {
+    Hyp h;
+    load_hyp(h, p, c15, *x, 0);
+    double out[5], F[5][5];
+    if (!propagate_state(*cfg, h.p, h.x, x_new, out, F, nullptr)) return 0;
+    if (F25) std::memcpy(F25, F, sizeof F);
+    if (!propagate(*cfg, h, x_new, nullptr, nullptr)) return 0;
+    std::memcpy(p, h.p, sizeof h.p);
+    store_cov(h, c15);
+    *x = h.x;
+    return 1;
+}
+
+int orc_rotate(const orc_config* cfg, double p[5], double c15[15], double* x, double beta, double* J25) {
+    Hyp h;
+    load_hyp(h, p, c15, *x, 0);
+    double out[5], J[5][5], xn;
+    if (!rotate_state(*cfg, h.p, h.x, beta, out, &xn, J, nullptr)) return 0;
+    if (J25) std::memcpy(J25, J, sizeof J);
+    if (!rotate(*cfg, h, beta, nullptr, nullptr)) return 0;
+    std::memcpy(p, h.p, sizeof h.p);
+    store_cov(h, c15);
+    *x = h.x;
+    return 1;
+}
+
+int orc_propagate_to_layer(const orc_config* cfg, double p[5], double c15[15], double* x, int32_t* sector, double X) {
+    Hyp h;
+    load_hyp(h, p, c15, *x, *sector);
+    if (!propagate_to_layer(*cfg, h, X, nullptr, nullptr)) return 0;
+    std::memcpy(p, h.p, sizeof h.p);
+    store_cov(h, c15);
+    *x = h.x;
+    *sector = h.sector;
+    return 1;
+}
+
+// Kalman update with (ym, zm); returns the chi2 increment
+double orc_update(const orc_config* cfg, double p[5], double c15[15], double ym, double zm) {
+    Hyp h;
+    load_hyp(h, p, c15, 0.0, 0);
+    const double c2 = kalman_update(*cfg, h, ym, zm);
+    std::memcpy(p, h.p, sizeof h.p);
+    store_cov(h, c15);
+    return c2;
+}
+
+// road half-widths and tan(phi) of a state: out = (road_y, road_z, tanphi, Sinv00, Sinv01, Sinv11)
+void orc_road(const orc_config* cfg, const double p[5], const double c15[15], double out[6]) {
+    Hyp h;
+    load_hyp(h, p, c15, 0.0, 0);
+    const Road rd = make_road(*cfg, h);
+    out[0] = rd.road_y; out[1] = rd.road_z; out[2] = rd.tanphi;
+    out[3] = rd.Sinv[0][0]; out[4] = rd.Sinv[0][1]; out[5] = rd.Sinv[1][1];
+}
+
+// accepted candidates of one state at one layer; returns their number (<= cap written)
+int orc_candidates(const orc_config* cfg, const float* y, const float* z, const float* dydx, const int32_t* chamber,
+                   int64_t n, const double p[5], const double c15[15], int sector, int layer, int brute,
+                   int32_t* out_index, double* out_chi2, int cap) {
+    Store st;
+    build_store(*cfg, y, z, dydx, chamber, n, !brute, st);
+    Hyp h;
+    load_hyp(h, p, c15, cfg->layer_x[layer], sector);
+    const Road rd = make_road(*cfg, h);
+    std::vector<Cand> cands;
+    find_candidates(*cfg, st, h, layer, rd, cands, nullptr, nullptr, nullptr);
+    std::sort(cands.begin(), cands.end(), [](const Cand& a, const Cand& b) { return a.index < b.index; });
+    for (int k = 0; k < (int)cands.size() && k < cap; ++k) {
+        out_index[k] = cands[k].index;
+        out_chi2[k] = cands[k].chi2inc;
+    }
+    return (int)cands.size();
+}
+
+// the whole step for n_trk tracks (float32 inputs exactly as the CUDA path receives them).
+// par: 5 x n_trk, cov: 15 x n_trk (SoA, row = component).  Outputs are double / int32 SoA:
+// out_idx 6 x n_trk, out_par 5 x n_trk, out_cov 15 x n_trk.  brute != 0 ignores the sorted
+// index and loops over all tracklets of the (sector, layer).  counters: n_prop, n_rot,
+// n_road, n_cand, n_upd, n_scanned.  seconds: index build, matching.
+int orc_match(const orc_config* cfg, const float* tl_y, const float* tl_z, const float* tl_dydx,
+              const int32_t* tl_chamber, int64_t n_tl, const float* par, const float* cov, const float* x,
+              const int32_t* sector, int64_t n_trk, int brute, int n_threads, int32_t* out_idx, double* out_par,
+              double* out_cov, double* out_x, int32_t* out_sector, double* out_chi2, int32_t* out_n_matched,
+              int32_t* out_n_evals, double* out_margin, int64_t counters[6], double seconds[2]) {
+    if (cfg->n_layers > kMaxLayers || cfg->n_hyp < 1) return -1;
+    const auto t0 = std::chrono::steady_clock::now();
+    Store st;
+    build_store(*cfg, tl_y, tl_z, tl_dydx, tl_chamber, n_tl, !brute, st);
+    const auto t1 = std::chrono::steady_clock::now();
+    Counters total;
+#ifdef _OPENMP
+    if (n_threads > 0) omp_set_num_threads(n_threads);
+#endif
+#pragma omp parallel
+    {
+        Counters local;
+#pragma omp for schedule(dynamic, 256)
+        for (int64_t i = 0; i < n_trk; ++i) {
+            double p[5], c15[15];
+            for (int k = 0; k < 5; ++k) p[k] = par[k * n_trk + i];
+            for (int k = 0; k < 15; ++k) c15[k] = cov[k * n_trk + i];
+            Hyp seed;
+            load_hyp(seed, p, c15, x[i], sector[i]);
+            seed.alive = std::fabs(p[2]) < cfg->max_snp && sector[i] >= 0 && sector[i] < cfg->n_sectors;
+            TrackResult res;
+            match_track(*cfg, st, seed, res, &local);
+            const Hyp& b = res.best;
+            for (int l = 0; l < kMaxLayers; ++l) out_idx[l * n_trk + i] = (l < cfg->n_layers) ? b.idx[l] : -1;
+            for (int k = 0; k < 5; ++k) out_par[k * n_trk + i] = b.p[k];
+            store_cov(b, c15);
+            for (int k = 0; k < 15; ++k) out_cov[k * n_trk + i] = c15[k];
+            out_x[i] = b.x;
+            out_sector[i] = b.sector;
+            out_chi2[i] = b.chi2;
+            out_n_matched[i] = b.n_matched;
+            if (out_n_evals) out_n_evals[i] = res.n_evals;
+            if (out_margin) out_margin[i] = res.margin;
+        }
+#pragma omp critical
+        {
+            total.n_prop += local.n_prop; total.n_rot += local.n_rot; total.n_road += local.n_road;
+            total.n_cand += local.n_cand; total.n_upd += local.n_upd; total.n_scanned += local.n_scanned;
+        }
+    }
+    const auto t2 = std::chrono::steady_clock::now();
+    if (counters) {
+        counters[0] = total.n_prop; counters[1] = total.n_rot; counters[2] = total.n_road;
+        counters[3] = total.n_cand; counters[4] = total.n_upd; counters[5] = total.n_scanned;
+    }
+    if (seconds) {
+        seconds[0] = std::chrono::duration<double>(t1 - t0).count();
+        seconds[1] = std::chrono::duration<double>(t2 - t1).count();
+    }
+    return 0;
+}
+
+int orc_max_threads(void) {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+}  // extern "C"

@@ -1,0 +1,305 @@
+"""Seeded synthetic inputs for the online TRD tracking step (§3).
+
+This module serves BOTH the oracle's tests and the CUDA path's tests / bench.  It
+holds none of the method's arithmetic: no Kalman filter, no road, no chi2, no
+propagation Jacobian.  All it computes is where a *true* particle crosses the TRD
+planes, from the global circle through the origin (an independent derivation of
+the helix, see `_truth_at_plane`), plus the smearing and noise the configs of
+BASELINE.json describe.  The paper measured on ALICE Monte-Carlo and 2018 HLT data
+(PAPER.md:74, 80, 94); those are not available, so these inputs stand in for them
+with the paper's shapes: 18 sectors x 5 stacks x 6 layers, ~2000-5000
+tracks per central event, time frames of 500-1000 collisions
+(PAPER.md:86, 90), >= 450k tracks per map.
+
+Recipe (every draw in float64, cast to float32 once at the end):
+  rng      numpy.random.Generator(PCG64(seed)), seed = 317400 + config number (1..5)
+  particle q = +-1, pT log-uniform [0.5, 20] GeV/c (config 4: 0.3 + Exp(0.5)),
+           eta uniform (-0.8, 0.8), tan(lambda) = sinh(eta), phi0 uniform [0, 2pi),
+           vertex at the origin
+  seed     true state where the helix crosses local x = 247 cm in the sector whose
+           |y| <= 247 tan(10 deg), smeared by N(0, diag(0.1, 0.1, 1e-3, 1e-3,
+           0.01 |q/pT|)^2); covariance = that diagonal
+  signal   per layer, with probability 0.9 and if |z| < 350 and |sin(phi)| < 0.95:
+           y + N(0, 0.04), z -> pad-row centre (8 cm rows), dy/dx = tan(phi) + N(0, 0.02)
+  noise    chamber uniform 0..539, y uniform in the chamber, z a uniform pad-row
+           centre of that stack, dy/dx uniform [-0.5, 0.5]
+  order    tracklets = signal ++ noise, then one seeded permutation
+"""
+from __future__ import annotations
+
+import dataclasses
+import math
+from typing import Dict, Optional
+
+import numpy as np
+
+# ---- geometry of the configs (BASELINE.json configs[0]) ---------------------------------
+N_SECTORS = 18
+N_STACKS = 5
+N_LAYERS = 6
+LAYER_X = (300.0, 313.0, 326.0, 338.0, 351.0, 364.0)
+X_SEED = 247.0
+Z_MAX = 350.0
+PAD_LENGTH = 8.0
+SECTOR_WIDTH = 2.0 * math.pi / N_SECTORS          # 20 degrees
+TAN_HALF_SECTOR = math.tan(0.5 * SECTOR_WIDTH)    # tan(10 degrees)
+KAPPA_PER_TESLA = -0.00299792458                  # curvature [1/cm] = this * Bz[T] * q/pT[c/GeV]
+N_ROWS = int(round(2 * (Z_MAX + 2.0) / PAD_LENGTH))  # 88 global pad rows, centres -348..+348
+
+SIGMA_SEED = (0.1, 0.1, 1e-3, 1e-3)               # y, z, sin(phi), tan(lambda); q/pT is relative
+REL_SIGMA_QPT = 0.01
+SIGMA_Y_TRACKLET = 0.04
+SIGMA_DYDX_TRACKLET = 0.02
+EFFICIENCY = 0.9
+MAX_SNP = 0.95
+NOISE_DYDX_RANGE = 0.5
+
+
+@dataclasses.dataclass(frozen=True)
+class WorkloadSpec:
+    """One of the five BASELINE.json configs (or a scaled / special variant of one)."""
+    name: str
+    number: int                 # 1..5; seed = 317400 + number
+    n_tracks: int
+    n_noise: int
+    n_hyp: int
+    n_sigma_road: float
+    pt_spectrum: str = "loguniform"   # or "exp"
+    batch: Optional[int] = None       # tracks per trd_match call (config 5: 500k)
+    bz: float = 0.5
+    # switches used by the oracle's pins (exact-recovery and pull tests)
+    smear_seed: bool = True
+    smear_tracklets: bool = True
+    exact_z: bool = False             # tracklet z = true z instead of the pad-row centre
+    efficiency: float = EFFICIENCY
+
+    @property
+    def seed(self) -> int:
+        return 317400 + self.number
+
+
+CONFIGS: Dict[str, WorkloadSpec] = {
+    "tiny": WorkloadSpec("tiny", 1, 1_000, 2_000, 1, 3.0),
+    "central": WorkloadSpec("central", 2, 5_000, 20_000, 1, 3.0),
+    "central8": WorkloadSpec("central8", 3, 5_000, 20_000, 8, 5.0),
+    "pileup": WorkloadSpec("pileup", 4, 25_000, 100_000, 4, 3.0, pt_spectrum="exp"),
+    "timeframe": WorkloadSpec("timeframe", 5, 2_000_000, 8_000_000, 4, 3.0, batch=500_000),
+}
+
+
+def scaled(spec: WorkloadSpec, n_tracks: int, name: Optional[str] = None) -> WorkloadSpec:
+    """Same generator, density per chamber preserved: noise scales with the track count."""
+    f = n_tracks / spec.n_tracks
+    return dataclasses.replace(spec, name=name or f"{spec.name}_x{n_tracks}", n_tracks=n_tracks,
+                               n_noise=int(round(spec.n_noise * f)),
+                               batch=None if spec.batch is None else min(spec.batch, n_tracks))
+
+
+def matcher_config(spec: WorkloadSpec) -> dict:
+    """The cuts and geometry of a config as a plain dict (field names of include/trdmatch.h).
+
+    Both the oracle wrapper and the CUDA binding turn this dict into their own struct.
+    """
+    return dict(
+        n_sectors=N_SECTORS, n_stacks=N_STACKS, n_layers=N_LAYERS,
+        layer_x=list(LAYER_X), z_max=Z_MAX, pad_length=PAD_LENGTH, bz_tesla=spec.bz,
+        sigma_y=SIGMA_Y_TRACKLET, sigma_z=PAD_LENGTH / math.sqrt(12.0),
+        sigma_dydx=SIGMA_DYDX_TRACKLET, n_sigma_road=spec.n_sigma_road, n_sigma_angle=4.0,
+        chi2_cut=15.0, chi2_penalty=15.0, max_snp=MAX_SNP, n_hyp=spec.n_hyp, ybin_width=0.0,
+    )
+
+
+# ---- pad rows and stacks (SURVEY.md §8(c).5 reading 12) ----------------------------------
+def pad_row_centre(z):
+    return PAD_LENGTH * (np.floor(np.asarray(z) / PAD_LENGTH) + 0.5)
+
+
+def stack_of_z(zc):
+    """Stack 0..4 of a pad-row centre: five equal 140 cm slices of [-350, 350]."""
+    width = 2.0 * Z_MAX / N_STACKS
+    return np.clip(np.floor((np.asarray(zc) + Z_MAX) / width), 0, N_STACKS - 1).astype(np.int64)
+
+
+def _rows_by_stack():
+    centres = PAD_LENGTH * (np.arange(N_ROWS) - N_ROWS // 2 + 0.5)
+    st = stack_of_z(centres)
+    return [centres[st == k] for k in range(N_STACKS)]
+
+
+# ---- truth: the global circle through the origin ----------------------------------------
+def _truth_at_plane(phi0, kappa, tanl, x_plane):
+    """Where the true particle first crosses the plane local-x = x_plane of its sector.
+
+    The particle leaves the origin with azimuth phi0; its xy projection is the circle of
+    signed curvature kappa (d(azimuth)/d(path) = kappa) through the origin, centre at
+    (-sin(phi0), cos(phi0))/kappa.  In a frame rotated by alpha the direction at the origin
+    is phi0 - alpha and the plane x' = X is met where sin(phi') = sin(phi0 - alpha) + kappa X
+    (chord of the circle), at y' = (cos(phi0 - alpha) - cos(phi'))/kappa after an arc of
+    length (phi' - (phi0 - alpha))/kappa.  The sector is the one whose |y'| <= X tan(10 deg).
+
+    Returns sector, y, z, sin(phi), ok  (ok = False where the circle does not reach).
+    """
+    n = phi0.shape[0]
+    # azimuth of the point of the circle at distance X/cos(.) ~ X from the origin: phi0 + asin(kappa rho / 2)
+    arg = np.clip(0.5 * kappa * x_plane, -1.0, 1.0)
+    az = np.mod(phi0 + np.arcsin(arg), 2.0 * np.pi)
+    guess = np.floor(az / SECTOR_WIDTH).astype(np.int64)
+    best = dict(sec=np.zeros(n, np.int64), y=np.full(n, np.nan), z=np.full(n, np.nan),
+                s=np.full(n, np.nan), ok=np.zeros(n, bool))
+    edge = x_plane * TAN_HALF_SECTOR
+    for d in (0, -1, 1):
+        sec = np.mod(guess + d, N_SECTORS)
+        alpha = (sec + 0.5) * SECTOR_WIDTH
+        ploc = np.mod(phi0 - alpha + np.pi, 2.0 * np.pi) - np.pi       # direction at the origin, local
+        s0 = np.sin(ploc)
+        c0 = np.cos(ploc)
+        s1 = s0 + kappa * x_plane
+        reach = (np.abs(s1) < 1.0) & (c0 > 0.0)
+        s1c = np.where(reach, s1, 0.0)
+        c1 = np.sqrt(1.0 - s1c * s1c)
+        straight = np.abs(kappa) < 1e-12
+        ksafe = np.where(straight, 1.0, kappa)
+        y = np.where(straight, x_plane * s0 / np.where(c0 > 0, c0, 1.0), (c0 - c1) / ksafe)
+        arc = np.where(straight, x_plane / np.where(c0 > 0, c0, 1.0), (np.arcsin(s1c) - ploc) / ksafe)
+        z = tanl * arc
+        take = reach & (np.abs(y) <= edge) & ~best["ok"]
+        best["sec"] = np.where(take, sec, best["sec"])
+        best["y"] = np.where(take, y, best["y"])
+        best["z"] = np.where(take, z, best["z"])
+        best["s"] = np.where(take, s1, best["s"])
+        best["ok"] |= take
+    return best["sec"], best["y"], best["z"], best["s"], best["ok"]
+
+
+def _draw_particles(rng, spec: WorkloadSpec, n: int):
+    q = np.where(rng.random(n) < 0.5, -1.0, 1.0)
+    if spec.pt_spectrum == "loguniform":
+        pt = np.exp(rng.uniform(math.log(0.5), math.log(20.0), n))
+    elif spec.pt_spectrum == "exp":
+        pt = 0.3 + rng.exponential(0.5, n)
+    else:
+        raise ValueError(spec.pt_spectrum)
+    eta = rng.uniform(-0.8, 0.8, n)
+    phi0 = rng.uniform(0.0, 2.0 * np.pi, n)
+    return q, pt, np.sinh(eta), phi0
+
+
+def generate(spec: WorkloadSpec) -> dict:
+    """Build the inputs of one config.  Deterministic: same spec -> identical bytes.
+
+    Returns a dict of numpy arrays:
+      tracks:    par (5, n) f32, cov (15, n) f32 lower-triangular, x (n,) f32, sector (n,) i32
+      tracklets: tl_y, tl_z, tl_dydx (m,) f32, tl_chamber (m,) i32, tl_label (m,) i32 (track id, -1 noise)
+      truth:     truth_par (5, n) f64 at the seed plane, truth_idx (n, 6) i32 = index of the
+                 track's own tracklet per layer in the permuted tracklet arrays (-1 = none),
+                 truth_last (n, 4) f64 = true (y, z, sin(phi), sector) at layer 5 (nan if not reached)
+    """
+    rng = np.random.Generator(np.random.PCG64(spec.seed))
+    n = spec.n_tracks
+    kfac = KAPPA_PER_TESLA * spec.bz
+
+    # 1. particles, redrawn in blocks of n until n of them reach x = 247 and layer 0 (draw order:
+    #    q, pT, eta, phi0 per block)
+    keep = {k: [] for k in ("q", "pt", "tanl", "phi0")}
+    have = 0
+    while have < n:
+        q, pt, tanl, phi0 = _draw_particles(rng, spec, max(n, 64))
+        kappa = kfac * q / pt
+        _, _, _, s_seed, ok_seed = _truth_at_plane(phi0, kappa, tanl, X_SEED)
+        _, _, _, s_l0, ok_l0 = _truth_at_plane(phi0, kappa, tanl, LAYER_X[0])
+        good = ok_seed & ok_l0 & (np.abs(s_seed) < MAX_SNP) & (np.abs(s_l0) < MAX_SNP)
+        for k, v in (("q", q), ("pt", pt), ("tanl", tanl), ("phi0", phi0)):
+            keep[k].append(v[good])
+        have += int(good.sum())
+    q, pt, tanl, phi0 = (np.concatenate(keep[k])[:n] for k in ("q", "pt", "tanl", "phi0"))
+    qpt = q / pt
+    kappa = kfac * qpt
+
+    # 2. seed state at x = 247 (+ smearing, draw order: 5 normals per track as one (n, 5) block)
+    sec, y, z, s, ok = _truth_at_plane(phi0, kappa, tanl, X_SEED)
+    assert ok.all()
+    truth_par = np.stack([y, z, s, tanl, qpt])
+    sig = np.stack([np.full(n, SIGMA_SEED[0]), np.full(n, SIGMA_SEED[1]), np.full(n, SIGMA_SEED[2]),
+                    np.full(n, SIGMA_SEED[3]), REL_SIGMA_QPT * np.abs(qpt)])
+    noise = rng.standard_normal((n, 5)).T
+    par = truth_par + (sig * noise if spec.smear_seed else 0.0)
+    cov = np.zeros((15, n))
+    for i in range(5):
+        cov[i * (i + 1) // 2 + i] = sig[i] ** 2
+
+    # 3. signal tracklets, layer by layer (draw order per layer: efficiency u, y normal, dy/dx normal)
+    sig_y, sig_z, sig_d, sig_ch, sig_lab, sig_lay = [], [], [], [], [], []
+    truth_last = np.full((n, 4), np.nan)
+    for lay, xl in enumerate(LAYER_X):
+        secl, yl, zl, sl, okl = _truth_at_plane(phi0, kappa, tanl, xl)
+        u = rng.random(n)
+        ny = rng.standard_normal(n)
+        nd = rng.standard_normal(n)
+        with np.errstate(invalid="ignore"):
+            present = okl & (np.abs(zl) < Z_MAX) & (np.abs(sl) < MAX_SNP) & (u < spec.efficiency)
+        if lay == N_LAYERS - 1:
+            truth_last[okl] = np.stack([yl, zl, sl, secl.astype(float)], axis=1)[okl]
+        idx = np.nonzero(present)[0]
+        yy = yl[idx] + (SIGMA_Y_TRACKLET * ny[idx] if spec.smear_tracklets else 0.0)
+        zc = pad_row_centre(zl[idx])
+        zz = zl[idx] if spec.exact_z else zc
+        tanphi = sl[idx] / np.sqrt(1.0 - sl[idx] ** 2)
+        dd = tanphi + (SIGMA_DYDX_TRACKLET * nd[idx] if spec.smear_tracklets else 0.0)
+        sig_y.append(yy); sig_z.append(zz); sig_d.append(dd)
+        sig_ch.append(secl[idx] * (N_STACKS * N_LAYERS) + stack_of_z(zc) * N_LAYERS + lay)
+        sig_lab.append(idx); sig_lay.append(np.full(idx.shape[0], lay))
+
+    # 4. noise tracklets (draw order: chamber, y, row pick, dy/dx)
+    m_noise = spec.n_noise
+    ch = rng.integers(0, N_SECTORS * N_STACKS * N_LAYERS, m_noise)
+    lay_n = ch % N_LAYERS
+    st_n = (ch // N_LAYERS) % N_STACKS
+    xl_n = np.asarray(LAYER_X)[lay_n]
+    y_n = rng.uniform(-1.0, 1.0, m_noise) * xl_n * TAN_HALF_SECTOR
+    rows = _rows_by_stack()
+    pick = rng.random(m_noise)
+    z_n = np.empty(m_noise)
+    for k in range(N_STACKS):
+        sel = st_n == k
+        z_n[sel] = rows[k][np.minimum((pick[sel] * len(rows[k])).astype(np.int64), len(rows[k]) - 1)]
+    d_n = rng.uniform(-NOISE_DYDX_RANGE, NOISE_DYDX_RANGE, m_noise)
+
+    # 5. concatenate and permute
+    tl_y = np.concatenate(sig_y + [y_n]); tl_z = np.concatenate(sig_z + [z_n])
+    tl_d = np.concatenate(sig_d + [d_n]); tl_ch = np.concatenate(sig_ch + [ch])
+    tl_lab = np.concatenate(sig_lab + [np.full(m_noise, -1)])
+    tl_lay = np.concatenate(sig_lay + [lay_n])
+    m = tl_y.shape[0]
+    perm = rng.permutation(m)
+    tl_y, tl_z, tl_d, tl_ch, tl_lab, tl_lay = (a[perm] for a in (tl_y, tl_z, tl_d, tl_ch, tl_lab, tl_lay))
+    truth_idx = np.full((n, N_LAYERS), -1, np.int32)
+    is_sig = tl_lab >= 0
+    truth_idx[tl_lab[is_sig], tl_lay[is_sig]] = np.nonzero(is_sig)[0].astype(np.int32)
+
+    return dict(
+        spec=spec,
+        par=np.ascontiguousarray(par, np.float32), cov=np.ascontiguousarray(cov, np.float32),
+        x=np.full(n, X_SEED, np.float32), sector=sec.astype(np.int32),
+        tl_y=tl_y.astype(np.float32), tl_z=tl_z.astype(np.float32), tl_dydx=tl_d.astype(np.float32),
+        tl_chamber=tl_ch.astype(np.int32), tl_label=tl_lab.astype(np.int32),
+        truth_par=truth_par, truth_idx=truth_idx, truth_last=truth_last,
+    )
+
+
+def efficiency_purity(out_idx: np.ndarray, data: dict) -> dict:
+    """The paper's two quality definitions on the generator's truth labels.
+
+    efficiency = fraction of tracks matched to >= 2 correct tracklets;
+    purity     = fraction of tracks with >= 2 attached tracklets that have no fake attached.
+    """
+    lab = data["tl_label"]
+    attached = out_idx >= 0
+    lab_of = np.where(attached, lab[np.where(attached, out_idx, 0)], -2)
+    own = np.arange(out_idx.shape[0])[:, None]
+    correct = (lab_of == own).sum(axis=1)
+    fake = (attached & (lab_of != own)).sum(axis=1)
+    n_att = attached.sum(axis=1)
+    ge2 = n_att >= 2
+    return dict(efficiency=float((correct >= 2).mean()),
+                purity=float(((fake == 0) & ge2).sum() / max(int(ge2.sum()), 1)),
+                frac_ge2=float(ge2.mean()))
