@@ -1,0 +1,156 @@
+/* trdmatch.h -- C ABI of the B200-native online TRD tracking step of arXiv 2003.03174.
+ *
+ * The operation: PAPER.md section 3 (L46-66) and Fig. 2 (L40).  ITS-TPC seed tracks
+ * (y, z, sin(phi), tan(lambda), q/pT with a 5x5 covariance) are extrapolated to each of the
+ * TRD layers, the TRD tracklets inside a search road derived from the track
+ * covariance are scored by a chi2 built from y and z only, tracklets whose
+ * inclination is more than n_sigma_angle sigma off the track inclination are excluded
+ * (PAPER.md:60), the best n_hyp hypotheses per layer are kept (Fig. 2) and updated
+ * with a Kalman filter.  The paper prints no equation for any of this; the
+ * readings taken are listed in DESIGN.md ("Readings", R1..R23).
+ *
+ * Conventions: cm, Tesla, GeV/c.  Sector frame s is rotated by (s + 1/2) * 2pi/n_sectors about
+ * the beam axis; the state at local x is (y, z, sin(phi), tan(lambda), q/pT); curvature
+ * kappa = -0.00299792458 * bz_tesla * q/pT per cm.  A covariance is 15 floats, the lower
+ * triangle row by row: yy, zy, zz, sy, sz, ss, ty, tz, ts, tt, cy, cz, cs, ct, cc.
+ * chamber = sector * (n_stacks * n_layers) + stack * n_layers + layer.
+ *
+ * All arrays are structure-of-arrays, one contiguous array per component.  Pointers named
+ * d_* or placed in trd_tracks_in / trd_tracks_out are DEVICE pointers owned by the caller
+ * (the Python binding allocates them with torch); the *_host entry points take HOST pointers
+ * instead and do the copies themselves.  `stream` is a cudaStream_t passed as void* (NULL =
+ * the legacy default stream).  Device entry points are asynchronous on `stream` and never
+ * call cudaDeviceSynchronize; they synchronise `stream` only when an internal buffer has to
+ * grow.  Calls on one handle are not thread-safe; several handles may coexist.
+ *
+ * Every int-returning call returns TRD_OK (0) or a negative trd_status; nothing throws or
+ * aborts.  trd_last_error() gives the text of the last failure on a handle.
+ * There is no CPU fallback: without a CUDA device trd_create fails with TRD_E_CUDA.
+ */
+#ifndef TRDMATCH_H_
+#define TRDMATCH_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define TRD_MAX_LAYERS 6
+#define TRD_MAX_HYP 8
+#define TRD_VERSION 100
+
+typedef enum trd_status {
+    TRD_OK = 0,
+    TRD_E_ARG = -1,    /* NULL pointer, bad size, bad config field */
+    TRD_E_CUDA = -2,   /* a CUDA runtime call failed (text in trd_last_error) */
+    TRD_E_NOMEM = -3,  /* device or host allocation failed */
+    TRD_E_STATE = -4   /* trd_match before any trd_load_tracklets */
+} trd_status;
+
+/* Geometry, field and cuts (BASELINE.json configs[0]; readings R2-R5, R8, R10-R12, R14).
+ * struct_size must be sizeof(trd_config). */
+typedef struct trd_config {
+    uint32_t struct_size;
+    int32_t n_sectors;               /* 18; 1..64 */
+    int32_t n_stacks;                /* 5; only used to decode `chamber` */
+    int32_t n_layers;                /* 6; 1..TRD_MAX_LAYERS */
+    int32_t n_hyp;                   /* N_candidates of PAPER.md:60; 1..TRD_MAX_HYP */
+    double layer_x[TRD_MAX_LAYERS];  /* local x of the layer planes, increasing */
+    double z_max;                    /* half length of the detector along z (350) */
+    double pad_length;               /* pad-row pitch along z (8) */
+    double bz_tesla;                 /* uniform solenoid field */
+    double sigma_y;                  /* tracklet y resolution (0.04) */
+    double sigma_z;                  /* tracklet z resolution (pad_length / sqrt(12)) */
+    double sigma_dydx;               /* tracklet inclination resolution (0.02) */
+    double n_sigma_road;             /* road half width in sigma (3 or 5) */
+    double n_sigma_angle;            /* inclination veto in sigma (4) */
+    double chi2_cut;                 /* per-layer chi2 increment cut (15) */
+    double chi2_penalty;             /* score added for a layer without tracklet (15) */
+    double max_snp;                  /* a hypothesis dies at |sin(phi)| >= max_snp (0.95) */
+    double ybin_width;               /* local-y bin width of the tracklet index; 0 = chosen per load */
+} trd_config;
+
+/* Input tracks of one batch: device pointers, each of length n_tracks. */
+typedef struct trd_tracks_in {
+    const float* par[5];    /* y, z, sin(phi), tan(lambda), q/pT at local x */
+    const float* cov[15];   /* lower triangle, order above */
+    const float* x;         /* local x of the state (247 in the configs) */
+    const int32_t* sector;  /* sector frame of the state, 0..n_sectors-1 */
+} trd_tracks_in;
+
+/* Output of one batch: caller-allocated device pointers, each of length n_tracks.  The best
+ * hypothesis after the last layer: tracklet_idx[l] is the position of the attached tracklet
+ * in the arrays given to trd_load_tracklets (-1 = none); state, covariance, x and sector are
+ * those at the last layer plane the hypothesis reached alive; chi2 is the sum of the chi2
+ * increments (no penalties).  n_cand_evals (may be NULL) counts, over all layers and
+ * hypotheses of the track, the tracklets found inside both road windows and past the
+ * inclination veto.  out->par[k] may alias in->par[k] (same for cov, x, sector). */
+typedef struct trd_tracks_out {
+    int32_t* tracklet_idx[TRD_MAX_LAYERS];
+    float* par[5];
+    float* cov[15];
+    float* x;
+    int32_t* sector;
+    float* chi2;
+    int32_t* n_matched;
+    int32_t* n_cand_evals;
+} trd_tracks_out;
+
+/* What trd_load_tracklets built (for tests and traffic accounting). */
+typedef struct trd_index_info {
+    int64_t n_tracklets;   /* tracklets given */
+    int32_t n_zrows;       /* z rows per (sector, layer) */
+    int32_t n_ybins;       /* y bins per z row (power of two) */
+    int64_t n_bins;        /* n_sectors * n_layers * n_zrows * n_ybins */
+    double ybin_width;     /* cm */
+    int32_t key_bits;      /* radix-sorted key width */
+    int32_t n_passes;      /* 8-bit radix passes */
+} trd_index_info;
+
+typedef struct trd_handle trd_handle;
+
+int trd_version(void);
+
+/* Validates and copies *cfg, derives the float32 constants.  Allocates nothing proportional
+ * to data.  The library owns *out until trd_destroy. */
+int trd_create(const trd_config* cfg, trd_handle** out);
+
+/* Frees everything the handle owns (synchronises the device first).  NULL is a no-op. */
+void trd_destroy(trd_handle* h);
+
+/* Builds the tracklet index on the device (north_star: "device-side sort and index by chamber
+ * and local-y bin"; PAPER.md:50 for the 18 x 5 x 6 segmentation): key = ((sector, layer), z row,
+ * y bin) -> stable LSD radix sort of (key, position) -> gather of (y, z, dy/dx, position) into
+ * the sorted store -> first-position table per bin.  Tracklets with a chamber outside
+ * 0..n_chambers-1 or a non-finite y or z are never candidates.  Replaces any previous index.
+ * The four input arrays (length n, n >= 0) are only read, and only until the work queued on
+ * `stream` by this call has run. */
+int trd_load_tracklets(trd_handle* h, const float* d_y, const float* d_z, const float* d_dydx,
+                       const int32_t* d_chamber, int64_t n, void* stream);
+
+/* The tracking step for one batch (n_tracks >= 0) against the loaded index. */
+int trd_match(trd_handle* h, const trd_tracks_in* in, const trd_tracks_out* out, int64_t n_tracks,
+              void* stream);
+
+/* Same two calls with HOST arrays: the library copies the inputs to its own device buffers
+ * on `stream`, runs the same kernels, copies the outputs back and synchronises `stream`
+ * before returning (trd_load_tracklets_host returns without waiting for the kernels). */
+int trd_load_tracklets_host(trd_handle* h, const float* y, const float* z, const float* dydx,
+                            const int32_t* chamber, int64_t n, void* stream);
+int trd_match_host(trd_handle* h, const trd_tracks_in* in_host, const trd_tracks_out* out_host,
+                   int64_t n_tracks, void* stream);
+
+/* Diagnostics.  trd_copy_index copies the sorted tracklet positions (n_tracklets int32), the
+ * sorted keys (n_tracklets uint32) and the first-position table (n_bins + 1 int32) to HOST
+ * arrays (any may be NULL) after synchronising `stream`. */
+int trd_get_index_info(const trd_handle* h, trd_index_info* info);
+int trd_copy_index(trd_handle* h, int32_t* sorted_pos, uint32_t* sorted_key, int32_t* bin_first, void* stream);
+const char* trd_last_error(const trd_handle* h);
+int64_t trd_device_bytes(const trd_handle* h);   /* device memory currently owned by the handle */
+int64_t trd_kernel_launches(const trd_handle* h); /* kernels launched through this handle so far */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TRDMATCH_H_ */

@@ -1,0 +1,264 @@
+// api.cu -- the extern "C" entry points declared in include/trdmatch.h: argument checks,
+// constants, buffer ownership, the host-buffer variants.  All arithmetic of the method lives in
+// index.cu and match.cu.
+#include <math.h>
+#include <string.h>
+
+#include <new>
+
+#include "trd_internal.cuh"
+
+namespace {
+
+int fail(trd_handle* h, int code, const std::string& what) {
+    if (h) h->err = what;
+    return code;
+}
+
+int fail_cuda(trd_handle* h, cudaError_t e, const char* where) {
+    cudaGetLastError();   // clear the sticky-less error state
+    const int code = (e == cudaErrorMemoryAllocation) ? TRD_E_NOMEM : TRD_E_CUDA;
+    return fail(h, code, std::string(where) + ": " + cudaGetErrorString(e));
+}
+
+bool derive_params(const trd_config& c, trd::MatchParams& mp) {
+    memset(&mp, 0, sizeof mp);
+    trd::IndexGeom& g = mp.g;
+    g.n_sectors = c.n_sectors;
+    g.n_layers = c.n_layers;
+    g.per_sector = c.n_stacks * c.n_layers;
+    g.n_chambers = c.n_sectors * g.per_sector;
+    mp.n_hyp = c.n_hyp;
+    const double half = M_PI / c.n_sectors;
+    for (int l = 0; l < c.n_layers; ++l) {
+        mp.layer_x[l] = (float)c.layer_x[l];
+        mp.edge[l] = (float)(c.layer_x[l] * tan(half));
+    }
+    mp.b = (float)(-0.00299792458 * c.bz_tesla);
+    const double cb = cos(2.0 * half), sb = sin(2.0 * half);
+    mp.cb_hi = (float)cb;
+    mp.cb_lo = (float)(cb - (double)mp.cb_hi);
+    mp.sb_hi = (float)sb;
+    mp.sb_lo = (float)(sb - (double)mp.sb_hi);
+    mp.sig_y2 = (float)(c.sigma_y * c.sigma_y);
+    mp.sig_z2 = (float)(c.sigma_z * c.sigma_z);
+    mp.n_sigma_road = (float)c.n_sigma_road;
+    mp.half_pad = (float)(0.5 * c.pad_length);
+    mp.veto = (float)(c.n_sigma_angle * c.sigma_dydx);
+    mp.chi2_cut = (float)c.chi2_cut;
+    mp.chi2_penalty = (float)c.chi2_penalty;
+    mp.max_snp = (float)c.max_snp;
+    return true;
+}
+
+const char* check_config(const trd_config& c) {
+    if (c.struct_size != sizeof(trd_config)) return "trd_config.struct_size does not match this library";
+    if (c.n_sectors < 1 || c.n_sectors > 64) return "n_sectors out of range";
+    if (c.n_stacks < 1 || c.n_stacks > 64) return "n_stacks out of range";
+    if (c.n_layers < 1 || c.n_layers > TRD_MAX_LAYERS) return "n_layers out of range";
+    if (c.n_hyp < 1 || c.n_hyp > TRD_MAX_HYP) return "n_hyp out of range";
+    for (int l = 0; l < c.n_layers; ++l) {
+        if (!(c.layer_x[l] > 0.0) || !isfinite(c.layer_x[l])) return "layer_x must be positive";
+        if (l > 0 && !(c.layer_x[l] > c.layer_x[l - 1])) return "layer_x must increase";
+    }
+    if (!(c.z_max > 0.0) || !(c.pad_length > 0.0)) return "z_max and pad_length must be positive";
+    if (c.z_max / c.pad_length > 4096.0) return "too many pad rows";
+    if (!isfinite(c.bz_tesla)) return "bz_tesla not finite";
+    if (!(c.sigma_y > 0.0) || !(c.sigma_z > 0.0) || !(c.sigma_dydx > 0.0)) return "sigmas must be positive";
+    if (!(c.n_sigma_road > 0.0) || !(c.n_sigma_angle > 0.0)) return "n_sigma_* must be positive";
+    if (!(c.chi2_cut > 0.0) || !(c.chi2_penalty >= 0.0)) return "chi2_cut / chi2_penalty out of range";
+    if (!(c.max_snp > 0.0) || !(c.max_snp < 1.0)) return "max_snp must be in (0, 1)";
+    if (!(c.ybin_width >= 0.0)) return "ybin_width must be >= 0";
+    return nullptr;
+}
+
+void release(trd::Buffer& b) {
+    if (b.p) cudaFree(b.p);
+    b.p = nullptr;
+    b.bytes = 0;
+}
+
+constexpr int kInArrays = 5 + 15 + 1 + 1;                    // par, cov, x, sector
+constexpr int kOutArrays = TRD_MAX_LAYERS + 5 + 15 + 5;      // idx, par, cov, x, sector, chi2, n_matched, n_cand_evals
+
+}  // namespace
+
+extern "C" {
+
+int trd_version(void) { return TRD_VERSION; }
+
+int trd_create(const trd_config* cfg, trd_handle** out) {
+    if (!cfg || !out) return TRD_E_ARG;
+    *out = nullptr;
+    if (check_config(*cfg)) return TRD_E_ARG;
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return TRD_E_CUDA;                                   // no device: there is no CPU fallback
+    }
+    trd_handle* h = new (std::nothrow) trd_handle();
+    if (!h) return TRD_E_NOMEM;
+    h->cfg = *cfg;
+    h->device = dev;
+    derive_params(h->cfg, h->mp);
+    cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, dev);
+    *out = h;
+    return TRD_OK;
+}
+
+void trd_destroy(trd_handle* h) {
+    if (!h) return;
+    cudaDeviceSynchronize();
+    release(h->store);
+    for (int s = 0; s < 2; ++s) {
+        release(h->key[s]);
+        release(h->val[s]);
+    }
+    release(h->tile_hist);
+    release(h->digit_tot);
+    release(h->bin_first);
+    release(h->stage_tl);
+    release(h->stage_in);
+    release(h->stage_out);
+    delete h;
+}
+
+int trd_load_tracklets(trd_handle* h, const float* d_y, const float* d_z, const float* d_dydx,
+                       const int32_t* d_chamber, int64_t n, void* stream) {
+    if (!h) return TRD_E_ARG;
+    if (n < 0 || n > 0x7fffffff) return fail(h, TRD_E_ARG, "trd_load_tracklets: n out of range");
+    if (n > 0 && (!d_y || !d_z || !d_dydx || !d_chamber)) return fail(h, TRD_E_ARG, "trd_load_tracklets: NULL array");
+    const cudaError_t e = trd::build_index(h, d_y, d_z, d_dydx, d_chamber, n, (cudaStream_t)stream);
+    if (e != cudaSuccess) return fail_cuda(h, e, "trd_load_tracklets");
+    return TRD_OK;
+}
+
+int trd_match(trd_handle* h, const trd_tracks_in* in, const trd_tracks_out* out, int64_t n_tracks, void* stream) {
+    if (!h) return TRD_E_ARG;
+    if (!in || !out || n_tracks < 0) return fail(h, TRD_E_ARG, "trd_match: NULL struct or negative n_tracks");
+    if (!h->index_loaded) return fail(h, TRD_E_STATE, "trd_match: no tracklets loaded");
+    if (n_tracks == 0) return TRD_OK;
+    for (int k = 0; k < 5; ++k)
+        if (!in->par[k] || !out->par[k]) return fail(h, TRD_E_ARG, "trd_match: NULL par array");
+    for (int k = 0; k < 15; ++k)
+        if (!in->cov[k] || !out->cov[k]) return fail(h, TRD_E_ARG, "trd_match: NULL cov array");
+    for (int l = 0; l < TRD_MAX_LAYERS; ++l)
+        if (!out->tracklet_idx[l]) return fail(h, TRD_E_ARG, "trd_match: NULL tracklet_idx array");
+    if (!in->x || !in->sector || !out->x || !out->sector || !out->chi2 || !out->n_matched)
+        return fail(h, TRD_E_ARG, "trd_match: NULL array");
+    const cudaError_t e = trd::launch_match(h, *in, *out, n_tracks, (cudaStream_t)stream);
+    if (e != cudaSuccess) return fail_cuda(h, e, "trd_match");
+    return TRD_OK;
+}
+
+int trd_load_tracklets_host(trd_handle* h, const float* y, const float* z, const float* dydx,
+                            const int32_t* chamber, int64_t n, void* stream) {
+    if (!h) return TRD_E_ARG;
+    if (n < 0 || n > 0x7fffffff) return fail(h, TRD_E_ARG, "trd_load_tracklets_host: n out of range");
+    if (n > 0 && (!y || !z || !dydx || !chamber)) return fail(h, TRD_E_ARG, "trd_load_tracklets_host: NULL array");
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t bytes = (size_t)n * 4;
+    cudaError_t e = trd::reserve(h->stage_tl, 4 * bytes + 16, st);
+    if (e != cudaSuccess) return fail_cuda(h, e, "trd_load_tracklets_host");
+    char* base = (char*)h->stage_tl.p;
+    const void* src[4] = {y, z, dydx, chamber};
+    for (int k = 0; k < 4 && n > 0; ++k) {
+        e = cudaMemcpyAsync(base + k * bytes, src[k], bytes, cudaMemcpyHostToDevice, st);
+        if (e != cudaSuccess) return fail_cuda(h, e, "trd_load_tracklets_host: copy");
+    }
+    return trd_load_tracklets(h, (const float*)base, (const float*)(base + bytes), (const float*)(base + 2 * bytes),
+                              (const int32_t*)(base + 3 * bytes), n, stream);
+}
+
+int trd_match_host(trd_handle* h, const trd_tracks_in* in, const trd_tracks_out* out, int64_t n, void* stream) {
+    if (!h) return TRD_E_ARG;
+    if (!in || !out || n < 0) return fail(h, TRD_E_ARG, "trd_match_host: NULL struct or negative n_tracks");
+    if (!h->index_loaded) return fail(h, TRD_E_STATE, "trd_match_host: no tracklets loaded");
+    if (n == 0) return TRD_OK;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t bytes = (size_t)n * 4;
+    cudaError_t e = trd::reserve(h->stage_in, kInArrays * bytes, st);
+    if (e == cudaSuccess) e = trd::reserve(h->stage_out, kOutArrays * bytes, st);
+    if (e != cudaSuccess) return fail_cuda(h, e, "trd_match_host");
+    char* bi = (char*)h->stage_in.p;
+    char* bo = (char*)h->stage_out.p;
+    trd_tracks_in din;
+    trd_tracks_out dout;
+    const void* src[kInArrays];
+    void* dst[kOutArrays];
+    int a = 0;
+    for (int k = 0; k < 5; ++k) { src[a] = in->par[k]; din.par[k] = (const float*)(bi + a * bytes); ++a; }
+    for (int k = 0; k < 15; ++k) { src[a] = in->cov[k]; din.cov[k] = (const float*)(bi + a * bytes); ++a; }
+    src[a] = in->x; din.x = (const float*)(bi + a * bytes); ++a;
+    src[a] = in->sector; din.sector = (const int32_t*)(bi + a * bytes); ++a;
+    int b = 0;
+    for (int l = 0; l < TRD_MAX_LAYERS; ++l) { dst[b] = out->tracklet_idx[l]; dout.tracklet_idx[l] = (int32_t*)(bo + b * bytes); ++b; }
+    for (int k = 0; k < 5; ++k) { dst[b] = out->par[k]; dout.par[k] = (float*)(bo + b * bytes); ++b; }
+    for (int k = 0; k < 15; ++k) { dst[b] = out->cov[k]; dout.cov[k] = (float*)(bo + b * bytes); ++b; }
+    dst[b] = out->x; dout.x = (float*)(bo + b * bytes); ++b;
+    dst[b] = out->sector; dout.sector = (int32_t*)(bo + b * bytes); ++b;
+    dst[b] = out->chi2; dout.chi2 = (float*)(bo + b * bytes); ++b;
+    dst[b] = out->n_matched; dout.n_matched = (int32_t*)(bo + b * bytes); ++b;
+    dst[b] = out->n_cand_evals; dout.n_cand_evals = out->n_cand_evals ? (int32_t*)(bo + b * bytes) : nullptr; ++b;
+    for (int k = 0; k < kInArrays; ++k) {
+        if (!src[k]) return fail(h, TRD_E_ARG, "trd_match_host: NULL input array");
+        e = cudaMemcpyAsync(bi + k * bytes, src[k], bytes, cudaMemcpyHostToDevice, st);
+        if (e != cudaSuccess) return fail_cuda(h, e, "trd_match_host: copy in");
+    }
+    for (int k = 0; k < kOutArrays - 1; ++k)
+        if (!dst[k]) return fail(h, TRD_E_ARG, "trd_match_host: NULL output array");
+    const int rc = trd_match(h, &din, &dout, n, stream);
+    if (rc != TRD_OK) return rc;
+    for (int k = 0; k < kOutArrays; ++k) {
+        if (!dst[k]) continue;
+        e = cudaMemcpyAsync(dst[k], bo + k * bytes, bytes, cudaMemcpyDeviceToHost, st);
+        if (e != cudaSuccess) return fail_cuda(h, e, "trd_match_host: copy out");
+    }
+    e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return fail_cuda(h, e, "trd_match_host: synchronize");
+    return TRD_OK;
+}
+
+int trd_get_index_info(const trd_handle* h, trd_index_info* info) {
+    if (!h || !info) return TRD_E_ARG;
+    if (!h->index_loaded) return TRD_E_STATE;
+    info->n_tracklets = h->n_tracklets;
+    info->n_zrows = h->mp.g.nz;
+    info->n_ybins = 1 << h->mp.g.nb_shift;
+    info->n_bins = h->mp.g.n_bins;
+    info->ybin_width = h->ybin_width;
+    info->key_bits = h->key_bits;
+    info->n_passes = h->n_passes;
+    return TRD_OK;
+}
+
+int trd_copy_index(trd_handle* h, int32_t* sorted_pos, uint32_t* sorted_key, int32_t* bin_first, void* stream) {
+    if (!h) return TRD_E_ARG;
+    if (!h->index_loaded) return fail(h, TRD_E_STATE, "trd_copy_index: no tracklets loaded");
+    cudaStream_t st = (cudaStream_t)stream;
+    cudaError_t e = cudaStreamSynchronize(st);
+    const size_t n = (size_t)h->n_tracklets;
+    if (e == cudaSuccess && sorted_pos && n)
+        e = cudaMemcpy(sorted_pos, h->val[h->sorted_side].p, n * 4, cudaMemcpyDeviceToHost);
+    if (e == cudaSuccess && sorted_key && n)
+        e = cudaMemcpy(sorted_key, h->key[h->sorted_side].p, n * 4, cudaMemcpyDeviceToHost);
+    if (e == cudaSuccess && bin_first)
+        e = cudaMemcpy(bin_first, h->bin_first.p, ((size_t)h->mp.g.n_bins + 1) * 4, cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) return fail_cuda(h, e, "trd_copy_index");
+    return TRD_OK;
+}
+
+const char* trd_last_error(const trd_handle* h) { return h ? h->err.c_str() : "NULL handle"; }
+
+int64_t trd_device_bytes(const trd_handle* h) {
+    if (!h) return 0;
+    size_t t = h->store.bytes + h->tile_hist.bytes + h->digit_tot.bytes + h->bin_first.bytes + h->stage_tl.bytes +
+               h->stage_in.bytes + h->stage_out.bytes;
+    for (int s = 0; s < 2; ++s) t += h->key[s].bytes + h->val[s].bytes;
+    return (int64_t)t;
+}
+
+int64_t trd_kernel_launches(const trd_handle* h) { return h ? h->launches : 0; }
+
+}  // extern "C"

@@ -1,0 +1,287 @@
+// index.cu -- the tracklet index of trd_load_tracklets.
+//
+//   a1  tracklet_key     key = ((sector, layer), z row, y bin) from (chamber, z, y)
+//   a2  radix_*          stable LSD radix sort of (key, position), 8 bits per pass:
+//                        per-tile digit histogram -> per-digit scan over tiles -> stable scatter
+//       gather_store     sorted store: one float4 (y, z, dy/dx, position) per tracklet
+//   a3  bin_first        first sorted position of every bin (plus sentinel)
+//
+// north_star: "device-side sort and index by chamber and local-y bin ... a radix sort plus
+// per-chamber y-bin offsets"; the 18 x 5 x 6 segmentation is PAPER.md:50.  The key also
+// carries the z row (SURVEY.md 8(d).3 "design consequence"), and it uses (sector, layer)
+// rather than the chamber's stack, because the z window may straddle two stacks (reading R12).
+// All of it is HBM-streaming integer work; no tensor cores.
+#include "trd_internal.cuh"
+
+namespace trd {
+
+namespace {
+
+constexpr int kRadixBits = 8;
+constexpr int kRadix = 1 << kRadixBits;
+constexpr int kSortThreads = 256;
+constexpr int kSortWarps = kSortThreads / 32;
+constexpr int kItems = 16;                          // keys per thread and tile
+constexpr int kTile = kSortThreads * kItems;        // 4096 keys per tile
+
+__global__ void __launch_bounds__(256) tracklet_key(const float* __restrict__ y, const float* __restrict__ z,
+                                                    const int32_t* __restrict__ chamber, uint32_t* __restrict__ key,
+                                                    int64_t n, IndexGeom g) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const float yy = y[i], zz = z[i];
+    const int ch = chamber[i];
+    uint32_t k = g.n_bins;                          // unusable: behind every bin
+    if (ch >= 0 && ch < g.n_chambers && isfinite(yy) && isfinite(zz)) {
+        const int sector = ch / g.per_sector, layer = ch % g.n_layers;
+        const uint32_t cell = (uint32_t)(sector * g.n_layers + layer);
+        k = ((cell * (uint32_t)g.nz + (uint32_t)zrow_of(g, zz)) << g.nb_shift) + (uint32_t)ybin_of(g, yy);
+    }
+    key[i] = k;
+}
+
+// per-tile histogram of one digit; hist[d * n_tiles + tile]
+__global__ void __launch_bounds__(kSortThreads) radix_hist(const uint32_t* __restrict__ key, uint32_t* __restrict__ hist,
+                                                           int64_t n, int n_tiles, int shift) {
+    __shared__ uint32_t cnt[kRadix];
+    cnt[threadIdx.x] = 0;
+    __syncthreads();
+    const int64_t base = (int64_t)blockIdx.x * kTile;
+#pragma unroll
+    for (int r = 0; r < kItems; ++r) {
+        const int64_t i = base + r * kSortThreads + threadIdx.x;
+        if (i < n) atomicAdd(&cnt[(key[i] >> shift) & (kRadix - 1)], 1u);
+    }
+    __syncthreads();
+    hist[(size_t)threadIdx.x * n_tiles + blockIdx.x] = cnt[threadIdx.x];
+}
+
+__device__ inline uint32_t block_exclusive_scan(uint32_t v, uint32_t* warp_sums, uint32_t* total) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    uint32_t incl = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t t = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += t;
+    }
+    if (lane == 31) warp_sums[warp] = incl;
+    __syncthreads();
+    if (warp == 0) {
+        uint32_t w = (lane < (int)(blockDim.x >> 5)) ? warp_sums[lane] : 0u;
+        uint32_t wi = w;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t t = __shfl_up_sync(0xffffffffu, wi, o);
+            if (lane >= o) wi += t;
+        }
+        warp_sums[lane] = wi - w;                  // exclusive warp offsets; [31] unused beyond n warps
+        if (lane == 31) *total = wi;
+    }
+    __syncthreads();
+    return warp_sums[warp] + incl - v;
+}
+
+// one block per digit: exclusive scan of that digit's counts over the tiles, total to digit_tot[d]
+__global__ void __launch_bounds__(kSortThreads) radix_rowscan(uint32_t* __restrict__ hist, uint32_t* __restrict__ digit_tot,
+                                                              int n_tiles) {
+    __shared__ uint32_t warp_sums[32];
+    __shared__ uint32_t total;
+    uint32_t* row = hist + (size_t)blockIdx.x * n_tiles;
+    uint32_t carry = 0;
+    for (int t0 = 0; t0 < n_tiles; t0 += kSortThreads) {
+        const int t = t0 + threadIdx.x;
+        const uint32_t v = (t < n_tiles) ? row[t] : 0u;
+        const uint32_t ex = block_exclusive_scan(v, warp_sums, &total);
+        if (t < n_tiles) row[t] = carry + ex;
+        carry += total;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) digit_tot[blockIdx.x] = carry;
+}
+
+// stable scatter of one tile.  Order inside a tile is (warp, round, lane): warp w owns the
+// contiguous keys [w * kItems * 32, (w + 1) * kItems * 32) of the tile.
+__global__ void __launch_bounds__(kSortThreads) radix_scatter(const uint32_t* __restrict__ key_in,
+                                                              const uint32_t* __restrict__ val_in,
+                                                              uint32_t* __restrict__ key_out, uint32_t* __restrict__ val_out,
+                                                              const uint32_t* __restrict__ hist,
+                                                              const uint32_t* __restrict__ digit_tot, int64_t n, int n_tiles,
+                                                              int shift) {
+    __shared__ uint32_t warp_cnt[kSortWarps][kRadix];
+    __shared__ uint32_t digit_base[kRadix];
+    __shared__ uint32_t warp_sums[32];
+    __shared__ uint32_t total;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const uint32_t lt = (1u << lane) - 1u;
+#pragma unroll
+    for (int w = 0; w < kSortWarps; ++w) warp_cnt[w][threadIdx.x] = 0;
+    // global base of digit d for this tile = (keys with a smaller digit) + (same digit in earlier tiles)
+    const uint32_t ex = block_exclusive_scan(digit_tot[threadIdx.x], warp_sums, &total);   // syncs
+    digit_base[threadIdx.x] = ex + hist[(size_t)threadIdx.x * n_tiles + blockIdx.x];
+
+    const int64_t base = (int64_t)blockIdx.x * kTile + (int64_t)warp * (kItems * 32);
+    uint32_t k[kItems], v[kItems], rank[kItems];
+#pragma unroll
+    for (int r = 0; r < kItems; ++r) {
+        const int64_t i = base + r * 32 + lane;
+        const bool ok = i < n;
+        k[r] = ok ? key_in[i] : 0u;
+        v[r] = ok ? (val_in ? val_in[i] : (uint32_t)i) : 0u;
+    }
+#pragma unroll
+    for (int r = 0; r < kItems; ++r) {
+        const bool ok = base + r * 32 + lane < n;
+        const uint32_t d = (k[r] >> shift) & (kRadix - 1);
+        const uint32_t peers = __match_any_sync(0xffffffffu, ok ? d : (uint32_t)kRadix);
+        uint32_t prior = 0;
+        if (ok) prior = warp_cnt[warp][d];
+        __syncwarp();
+        rank[r] = prior + __popc(peers & lt);
+        if (ok && (peers & lt) == 0) warp_cnt[warp][d] = prior + __popc(peers);
+        __syncwarp();
+    }
+    __syncthreads();
+    {   // exclusive scan over the warps, per digit
+        uint32_t run = 0;
+#pragma unroll
+        for (int w = 0; w < kSortWarps; ++w) {
+            const uint32_t c = warp_cnt[w][threadIdx.x];
+            warp_cnt[w][threadIdx.x] = run;
+            run += c;
+        }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int r = 0; r < kItems; ++r) {
+        if (base + r * 32 + lane < n) {
+            const uint32_t d = (k[r] >> shift) & (kRadix - 1);
+            const uint32_t dst = digit_base[d] + warp_cnt[warp][d] + rank[r];
+            key_out[dst] = k[r];
+            val_out[dst] = v[r];
+        }
+    }
+}
+
+__global__ void __launch_bounds__(256) gather_store(const uint32_t* __restrict__ pos, const float* __restrict__ y,
+                                                    const float* __restrict__ z, const float* __restrict__ dydx,
+                                                    float4* __restrict__ store, int64_t n) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const uint32_t j = pos[i];
+    store[i] = make_float4(y[j], z[j], dydx[j], __uint_as_float(j));
+}
+
+// bin_first[b] = first sorted position whose key is >= b, for b = 0..n_bins
+__global__ void __launch_bounds__(256) bin_first_kernel(const uint32_t* __restrict__ key, int32_t* __restrict__ bin_first,
+                                                        int64_t n, uint32_t n_bins) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const uint32_t k = min(key[i], n_bins);
+    const int64_t lo = (i == 0) ? 0 : (int64_t)min(key[i - 1], n_bins) + 1;
+    for (int64_t b = lo; b <= (int64_t)k; ++b) bin_first[b] = (int32_t)i;
+    if (i == n - 1)
+        for (int64_t b = (int64_t)k + 1; b <= (int64_t)n_bins; ++b) bin_first[b] = (int32_t)n;
+}
+
+inline int ceil_log2(uint64_t v) {
+    int b = 0;
+    while ((1ull << b) < v) ++b;
+    return b;
+}
+
+}  // namespace
+
+#define TRD_TRY(expr)                              \
+    do {                                           \
+        cudaError_t e_ = (expr);                   \
+        if (e_ != cudaSuccess) return e_;          \
+    } while (0)
+
+cudaError_t reserve(Buffer& b, size_t bytes, cudaStream_t stream) {
+    if (bytes <= b.bytes) return cudaSuccess;
+    if (b.p) {
+        TRD_TRY(cudaStreamSynchronize(stream));
+        TRD_TRY(cudaFree(b.p));
+        b.p = nullptr;
+        b.bytes = 0;
+    }
+    const size_t want = bytes + bytes / 8 + 256;    // a little head room against regrowth
+    TRD_TRY(cudaMalloc(&b.p, want));
+    b.bytes = want;
+    return cudaSuccess;
+}
+
+cudaError_t build_index(trd_handle* h, const float* d_y, const float* d_z, const float* d_dydx,
+                        const int32_t* d_chamber, int64_t n, cudaStream_t stream) {
+    const trd_config& c = h->cfg;
+    IndexGeom& g = h->mp.g;
+    // ---- geometry of the bins for this load ----
+    const int n_cells = c.n_sectors * c.n_layers;
+    const int half_rows = (int)ceil(c.z_max / c.pad_length) + 1;
+    g.nz = 2 * half_rows;
+    g.z_off = (float)(half_rows * c.pad_length);
+    g.inv_pad = (float)(1.0 / c.pad_length);
+    const double x_out = c.layer_x[c.n_layers - 1];
+    const double y_half = x_out * tan(M_PI / c.n_sectors) * 1.02 + 1.0;
+    int shift;
+    if (c.ybin_width > 0.0) {
+        shift = ceil_log2((uint64_t)ceil(2.0 * y_half / c.ybin_width));
+    } else {
+        // about two tracklets per bin on average, y bins between 8 and 1024 per row
+        const double per_row = (double)n / ((double)n_cells * g.nz);
+        shift = ceil_log2((uint64_t)fmax(per_row / 2.0, 1.0));
+    }
+    if (shift < 3) shift = 3;
+    if (shift > 10) shift = 10;
+    while (shift > 0 && (uint64_t)n_cells * g.nz * (1ull << shift) >= (1ull << 31)) --shift;
+    g.nb_shift = shift;
+    g.y_half = (float)y_half;
+    g.inv_w = (float)((double)(1 << shift) / (2.0 * y_half));
+    g.n_bins = (uint32_t)n_cells * (uint32_t)g.nz * (1u << shift);
+    h->ybin_width = 2.0 * y_half / (double)(1 << shift);
+    h->key_bits = ceil_log2((uint64_t)g.n_bins + 1);
+    h->n_passes = (h->key_bits + kRadixBits - 1) / kRadixBits;
+    h->n_tracklets = n;
+    h->index_loaded = false;
+
+    TRD_TRY(reserve(h->bin_first, ((size_t)g.n_bins + 1) * sizeof(int32_t), stream));
+    if (n == 0) {
+        TRD_TRY(cudaMemsetAsync(h->bin_first.p, 0, ((size_t)g.n_bins + 1) * sizeof(int32_t), stream));
+        h->index_loaded = true;
+        return cudaSuccess;
+    }
+    const int n_tiles = (int)((n + kTile - 1) / kTile);
+    TRD_TRY(reserve(h->store, (size_t)n * sizeof(float4), stream));
+    for (int s = 0; s < 2; ++s) {
+        TRD_TRY(reserve(h->key[s], (size_t)n * sizeof(uint32_t), stream));
+        TRD_TRY(reserve(h->val[s], (size_t)n * sizeof(uint32_t), stream));
+    }
+    TRD_TRY(reserve(h->tile_hist, (size_t)kRadix * n_tiles * sizeof(uint32_t), stream));
+    TRD_TRY(reserve(h->digit_tot, kRadix * sizeof(uint32_t), stream));
+
+    const unsigned n_blk = (unsigned)((n + 255) / 256);
+    tracklet_key<<<n_blk, 256, 0, stream>>>(d_y, d_z, d_chamber, (uint32_t*)h->key[0].p, n, g);
+    h->launches++;
+    int side = 0;
+    for (int p = 0; p < h->n_passes; ++p) {
+        const int sh = p * kRadixBits;
+        const uint32_t* kin = (const uint32_t*)h->key[side].p;
+        const uint32_t* vin = (p == 0) ? nullptr : (const uint32_t*)h->val[side].p;
+        radix_hist<<<n_tiles, kSortThreads, 0, stream>>>(kin, (uint32_t*)h->tile_hist.p, n, n_tiles, sh);
+        radix_rowscan<<<kRadix, kSortThreads, 0, stream>>>((uint32_t*)h->tile_hist.p, (uint32_t*)h->digit_tot.p, n_tiles);
+        radix_scatter<<<n_tiles, kSortThreads, 0, stream>>>(kin, vin, (uint32_t*)h->key[side ^ 1].p,
+                                                           (uint32_t*)h->val[side ^ 1].p, (const uint32_t*)h->tile_hist.p,
+                                                           (const uint32_t*)h->digit_tot.p, n, n_tiles, sh);
+        h->launches += 3;
+        side ^= 1;
+    }
+    h->sorted_side = side;
+    gather_store<<<n_blk, 256, 0, stream>>>((const uint32_t*)h->val[side].p, d_y, d_z, d_dydx, (float4*)h->store.p, n);
+    bin_first_kernel<<<n_blk, 256, 0, stream>>>((const uint32_t*)h->key[side].p, (int32_t*)h->bin_first.p, n, g.n_bins);
+    h->launches += 2;
+    TRD_TRY(cudaGetLastError());
+    h->index_loaded = true;
+    return cudaSuccess;
+}
+
+}  // namespace trd

@@ -1,0 +1,94 @@
+// trd_internal.cuh -- shared declarations of the CUDA path (not part of the C ABI).
+// Nothing here is used by, or uses, anything under oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+
+#include "trdmatch.h"
+
+namespace trd {
+
+// ---- geometry of the tracklet index ----------------
+// bin key = (((sector * n_layers + layer) * nz + zrow) << nb_shift) + ybin
+struct IndexGeom {
+    int n_sectors, n_layers, per_sector, n_chambers;
+    int nz;            // z rows per (sector, layer)
+    int nb_shift;      // log2(y bins per z row)
+    float z_off, inv_pad;
+    float y_half, inv_w;
+    uint32_t n_bins;   // also the key of an unusable tracklet (sorts behind every bin)
+};
+
+__host__ __device__ inline int zrow_of(const IndexGeom& g, float z) {
+    float f = floorf((z + g.z_off) * g.inv_pad);
+    f = fminf(fmaxf(f, 0.0f), (float)(g.nz - 1));
+    return (int)f;
+}
+
+__host__ __device__ inline int ybin_of(const IndexGeom& g, float y) {
+    float f = floorf((y + g.y_half) * g.inv_w);
+    f = fminf(fmaxf(f, 0.0f), (float)((1 << g.nb_shift) - 1));
+    return (int)f;
+}
+
+// ---- constants of the match kernel, float32, derived in double on the host -------------------
+struct MatchParams {
+    IndexGeom g;
+    int n_hyp;
+    float layer_x[TRD_MAX_LAYERS];
+    float edge[TRD_MAX_LAYERS];      // layer_x * tan(pi / n_sectors): the sector edge in y
+    float b;                         // kappa = b * q/pT
+    float cb_hi, cb_lo, sb_hi, sb_lo;  // cos / sin of the sector width, split hi + lo
+    float sig_y2, sig_z2;
+    float n_sigma_road, half_pad;
+    float veto;                      // n_sigma_angle * sigma_dydx
+    float chi2_cut, chi2_penalty, max_snp;
+};
+
+struct Buffer {
+    void* p = nullptr;
+    size_t bytes = 0;
+};
+
+}  // namespace trd
+
+struct trd_handle {
+    trd_config cfg;
+    trd::MatchParams mp;
+    int device = 0;
+    int sm_count = 0;
+    bool index_loaded = false;
+    int64_t n_tracklets = 0;
+    int key_bits = 0, n_passes = 0;
+    double ybin_width = 0.0;
+    int64_t launches = 0;
+    std::string err;
+    // device buffers owned by the handle
+    trd::Buffer store;      // float4 per sorted tracklet: y, z, dy/dx, original position (bits)
+    trd::Buffer key[2];     // uint32 keys, ping-pong
+    trd::Buffer val[2];     // uint32 original positions, ping-pong
+    trd::Buffer tile_hist;  // [256][n_tiles] digit counts per tile
+    trd::Buffer digit_tot;  // [256]
+    trd::Buffer bin_first;  // [n_bins + 1]
+    int sorted_side = 0;    // which of key[]/val[] holds the sorted result
+    // staging for the *_host entry points
+    trd::Buffer stage_tl;   // tracklets
+    trd::Buffer stage_in;   // tracks in
+    trd::Buffer stage_out;  // tracks out
+};
+
+namespace trd {
+
+// returns cudaSuccess or the first error; counts launches into h->launches
+cudaError_t build_index(trd_handle* h, const float* d_y, const float* d_z, const float* d_dydx,
+                        const int32_t* d_chamber, int64_t n, cudaStream_t stream);
+cudaError_t launch_match(trd_handle* h, const trd_tracks_in& in, const trd_tracks_out& out, int64_t n,
+                         cudaStream_t stream);
+
+// grows b to at least `bytes` (contents lost); synchronises `stream` before freeing
+cudaError_t reserve(Buffer& b, size_t bytes, cudaStream_t stream);
+
+}  // namespace trd

@@ -1,0 +1,71 @@
+"""Element-by-element comparison of two results of the tracking step (plain numpy dicts).
+
+Holds none of the method's arithmetic and imports neither the CUDA binding nor the oracle: the
+caller passes `got` (the CUDA path's output) and `want` (the reference result, which also carries
+the per-track fragility `margin`).  Criteria (BASELINE.json north_star):
+
+  assignment  tracklet index identical per track and layer, except on tracks whose reference
+              margin (smallest relative distance of any discrete decision from its threshold,
+              rank gaps included) is below `eps_margin`;
+  parameters  |got - want| <= 1e-4 |want| or <= 1e-5, on tracks with identical assignment;
+  chi2        |got - want| <= 1e-3 |want| (+ chi2_atol), same tracks;
+  integers    n_matched, sector, x exact on tracks with identical assignment.
+"""
+from __future__ import annotations
+
+from typing import Dict
+
+import numpy as np
+
+PAR_RTOL = 1e-4
+PAR_ATOL = 1e-5
+CHI2_RTOL = 1e-3
+EPS_MARGIN = 1e-4
+
+
+def compare(got: Dict[str, np.ndarray], want: Dict[str, np.ndarray], eps_margin: float = EPS_MARGIN,
+            chi2_atol: float = 0.0, cov_rtol: float = 2e-3) -> dict:
+    n = want["x"].shape[0]
+    same = np.all(got["idx"][:, :n] == want["idx"], axis=0)
+    fragile = want["margin"] < eps_margin
+    mism = ~same
+    rep = dict(n_tracks=int(n), n_assign_mismatch=int(mism.sum()), n_fragile=int(fragile.sum()),
+               n_unexplained=int((mism & ~fragile).sum()))
+    rep["unexplained_tracks"] = np.nonzero(mism & ~fragile)[0][:20].tolist()
+    rep["max_margin_of_mismatch"] = float(want["margin"][mism].max()) if mism.any() else 0.0
+    s = same
+    gp = got["par"][:, :n].astype(np.float64)
+    dp = np.abs(gp - want["par"])
+    par_ok = (dp <= PAR_RTOL * np.abs(want["par"])) | (dp <= PAR_ATOL)
+    bad_par = s & ~np.all(par_ok, axis=0)
+    rep["n_par_bad"] = int(bad_par.sum())
+    rep["par_bad_tracks"] = np.nonzero(bad_par)[0][:20].tolist()
+    with np.errstate(divide="ignore", invalid="ignore"):
+        rel = np.where(s[None, :], dp / np.maximum(np.abs(want["par"]), PAR_ATOL / PAR_RTOL), 0.0)
+    rep["par_max_scaled_err"] = [float(v) for v in rel.max(axis=1)] if n else [0.0] * 5
+    dc = np.abs(got["chi2"][:n].astype(np.float64) - want["chi2"])
+    bad_chi2 = s & ~(dc <= CHI2_RTOL * np.abs(want["chi2"]) + chi2_atol)
+    rep["n_chi2_bad"] = int(bad_chi2.sum())
+    rep["chi2_bad_tracks"] = np.nonzero(bad_chi2)[0][:20].tolist()
+    with np.errstate(divide="ignore", invalid="ignore"):
+        r = np.where(s & (want["chi2"] > 0), dc / np.abs(want["chi2"]), 0.0)
+    rep["chi2_max_rel_err"] = float(r.max()) if n else 0.0
+    ints_ok = (got["n_matched"][:n] == want["n_matched"]) & (got["sector"][:n] == want["sector"]) & \
+              (got["x"][:n].astype(np.float64) == want["x"])
+    rep["n_int_bad"] = int((s & ~ints_ok).sum())
+    # covariance: scaled by sqrt(C_ii C_jj) of the reference
+    tri = [(i, j) for i in range(5) for j in range(i + 1)]
+    diag = np.stack([want["cov"][i * (i + 1) // 2 + i] for i in range(5)])
+    scale = np.stack([np.sqrt(np.abs(diag[i] * diag[j])) for i, j in tri])
+    dcov = np.abs(got["cov"][:, :n].astype(np.float64) - want["cov"])
+    with np.errstate(divide="ignore", invalid="ignore"):
+        rc = np.where(s[None, :] & (scale > 0), dcov / scale, 0.0)
+    rep["cov_max_scaled_err"] = float(rc.max()) if n else 0.0
+    rep["n_cov_bad"] = int((rc > cov_rtol).any(axis=0).sum())
+    if "n_evals" in got and "n_evals" in want:
+        rep["n_evals_got"] = int(got["n_evals"][:n].astype(np.int64).sum())
+        rep["n_evals_want"] = int(want["n_evals"].astype(np.int64).sum())
+        rep["n_evals_bad"] = int((s & ~fragile & (got["n_evals"][:n] != want["n_evals"])).sum())
+    rep["ok"] = (rep["n_unexplained"] == 0 and rep["n_par_bad"] == 0 and rep["n_chi2_bad"] == 0
+                 and rep["n_int_bad"] == 0 and rep["n_cov_bad"] == 0)
+    return rep
