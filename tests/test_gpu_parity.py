@@ -1,0 +1,202 @@
+"""The parity tests proper: the CUDA path (through the C ABI) against the oracle, element by element, on
+the same seeded inputs.  Criteria: BASELINE.json north_star, implemented in paper_2003_03174_b200.parity."""
+import dataclasses
+
+import numpy as np
+import pytest
+
+from oracle import oracle as O
+from paper_2003_03174_b200 import parity as P, workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2003_03174_b200 import binding, build
+    build.build()
+    return binding
+
+
+def run_gpu(B, cfg, data, batch=None, in_place=False):
+    import torch
+    dev = B.to_device(data)
+    n = data["x"].shape[0]
+    h = B.trd_create(cfg)
+    try:
+        B.trd_load_tracklets(h, dev["tl_y"], dev["tl_z"], dev["tl_dydx"], dev["tl_chamber"])
+        if batch is None:
+            out = B.alloc_tracks_out(n)
+            if in_place:
+                out["par"], out["cov"], out["x"], out["sector"] = dev["par"], dev["cov"], dev["x"], dev["sector"]
+            B.trd_match(h, dev, out)
+            torch.cuda.synchronize()
+            return B.to_numpy(out)
+        parts = []
+        for lo in range(0, n, batch):
+            hi = min(n, lo + batch)
+            part = dict(par=dev["par"][:, lo:hi].contiguous(), cov=dev["cov"][:, lo:hi].contiguous(),
+                        x=dev["x"][lo:hi].contiguous(), sector=dev["sector"][lo:hi].contiguous())
+            parts.append(B.to_numpy(B.trd_match(h, part)))
+        return {k: np.concatenate([p[k] for p in parts], axis=-1) for k in parts[0]}
+    finally:
+        B.trd_destroy(h)
+
+
+def assert_parity(rep, want):
+    assert rep["ok"], {k: v for k, v in rep.items()}
+    assert rep["n_evals_bad"] == 0
+    # flips are only tolerated on fragile tracks, and there must be few of those
+    assert rep["n_assign_mismatch"] <= rep["n_fragile"]
+
+
+@pytest.mark.parametrize("name", ["tiny", "central", "central8", "pileup"])
+def test_configs_1_to_4_full_parity(B, name):
+    spec = W.CONFIGS[name]; d = W.generate(spec); cfg = W.matcher_config(spec)
+    want = O.match(cfg, d)
+    got = run_gpu(B, cfg, d)
+    rep = P.compare(got, want)
+    assert_parity(rep, want)
+    assert rep["n_fragile"] < 0.02 * spec.n_tracks
+
+
+def test_config_5_scaled_down_in_batches(B):
+    """Config 5's generator and cuts (nHyp = 4, 3 sigma) at 100k tracks and 400k noise tracklets (tracklet
+    density 1/20 of the full config), matched as 4 batches against one loaded index, every track checked."""
+    spec = W.scaled(W.CONFIGS["timeframe"], 100_000)
+    d = W.generate(spec); cfg = W.matcher_config(spec)
+    want = O.match(cfg, d)
+    got = run_gpu(B, cfg, d, batch=spec.batch // 4)
+    assert_parity(P.compare(got, want), want)
+
+
+def test_dense_candidates_many_per_road(B):
+    """Few tracks in dense noise (12M noise tracklets = about 2/3 of the per-chamber density of the full
+    config 5): several in-road candidates per hypothesis and layer; all sub-warp widths (nHyp 1, 2, 3, 4, 8)."""
+    for n_hyp, road, n_noise in ((4, 3.0, 12_000_000), (8, 5.0, 12_000_000), (3, 3.0, 4_000_000),
+                                 (2, 3.0, 4_000_000), (1, 3.0, 4_000_000)):
+        spec = dataclasses.replace(W.CONFIGS["tiny"], name="dense", number=7, n_tracks=3000, n_noise=n_noise,
+                                   n_hyp=n_hyp, n_sigma_road=road)
+        d = W.generate(spec); cfg = W.matcher_config(spec)
+        want = O.match(cfg, d)
+        assert want["counters"]["n_cand"] > want["counters"]["n_road"]
+        got = run_gpu(B, cfg, d)
+        rep = P.compare(got, want)
+        assert_parity(rep, want)
+
+
+def test_config_5_full_size_sampled(B):
+    """BASELINE.json configs[4] at full size in the launch configuration bench.py times (one load of all
+    ~18.8M tracklets, four trd_match calls of 500k tracks); the oracle checks a sample of the tracks one
+    by one against the full tracklet set."""
+    spec = W.CONFIGS["timeframe"]; d = W.generate(spec); cfg = W.matcher_config(spec)
+    got = run_gpu(B, cfg, d, batch=spec.batch)
+    rng = np.random.default_rng(5)
+    starts = np.sort(rng.choice(spec.n_tracks - 2048, 8, replace=False))
+    n_checked = 0
+    for lo in starts.tolist() + [spec.n_tracks - 2048]:
+        hi = lo + 2048
+        want = O.match(cfg, d, lo=lo, hi=hi)
+        part = {k: v[..., lo:hi] for k, v in got.items()}
+        rep = P.compare(part, want)
+        assert_parity(rep, want)
+        n_checked += hi - lo
+    assert n_checked >= 18_000
+    # properties that hold at any size
+    att = got["idx"] >= 0
+    assert np.array_equal(att.sum(axis=0), got["n_matched"])
+    assert got["idx"].max() < d["tl_y"].shape[0]
+    lay = d["tl_chamber"][np.where(att, got["idx"], 0)] % 6
+    assert np.all(lay[att] == np.nonzero(att)[0])                          # layer l holds a layer-l tracklet
+    sec_tl = d["tl_chamber"][np.where(att, got["idx"], 0)] // 30
+    assert np.all(sec_tl[5][att[5]] == got["sector"][att[5]])              # last attached = final sector
+    assert np.all(got["chi2"] >= 0) and np.all(got["chi2"] < 15.0 * 6)
+    assert np.all(np.isfinite(got["par"])) and np.all(np.isfinite(got["cov"]))
+
+
+def test_edge_cases(B, base_cfg):
+    import torch
+    spec = W.CONFIGS["tiny"]; d = W.generate(spec); cfg = W.matcher_config(spec)
+    want = O.match(cfg, d)
+    # in-place outputs (out->par == in->par)
+    assert_parity(P.compare(run_gpu(B, cfg, d, in_place=True), want), want)
+    # ragged batches
+    assert_parity(P.compare(run_gpu(B, cfg, d, batch=333), want), want)
+    # dead seeds: |sin(phi)| >= max_snp, sector outside 0..17
+    d2 = dict(d); d2["par"] = d["par"].copy(); d2["par"][2, 0] = 0.96
+    d2["sector"] = d["sector"].copy(); d2["sector"][1] = 99; d2["sector"][2] = -1
+    want2 = O.match(cfg, d2); got2 = run_gpu(B, cfg, d2)
+    assert_parity(P.compare(got2, want2), want2)
+    assert got2["idx"][:, :3].max() == -1 and got2["n_matched"][:3].max() == 0
+    # no tracklets at all: every layer skipped, state = last alive propagation
+    d3 = dict(d); d3.update(tl_y=d["tl_y"][:0], tl_z=d["tl_z"][:0], tl_dydx=d["tl_dydx"][:0], tl_chamber=d["tl_chamber"][:0])
+    want3 = O.match(cfg, d3); got3 = run_gpu(B, cfg, d3)
+    assert_parity(P.compare(got3, want3), want3)
+    assert got3["idx"].max() == -1 and np.all(got3["x"] >= 247.0)
+    # zero tracks, and trd_match before any load
+    h = B.trd_create(cfg)
+    try:
+        dev = B.to_device(d)
+        with pytest.raises(B.TrdError) as e:
+            B.trd_match(h, dev)
+        assert e.value.code == B.TRD_E_STATE
+        B.trd_load_tracklets(h, dev["tl_y"], dev["tl_z"], dev["tl_dydx"], dev["tl_chamber"])
+        empty = dict(par=dev["par"][:, :0].contiguous(), cov=dev["cov"][:, :0].contiguous(),
+                     x=dev["x"][:0].contiguous(), sector=dev["sector"][:0].contiguous())
+        out = B.trd_match(h, empty)
+        assert out["x"].numel() == 0
+        with pytest.raises(B.TrdError) as e:                   # NULL array -> TRD_E_ARG, not a crash
+            import ctypes as C
+            tin, tout = B.TrdTracksIn(), B.TrdTracksOut()
+            rc = B.lib().trd_match(h, C.byref(tin), C.byref(tout), 5, None)
+            B._check(h, rc)
+        assert e.value.code == B.TRD_E_ARG
+        assert B.trd_device_bytes(h) > 0 and B.trd_kernel_launches(h) > 0
+    finally:
+        B.trd_destroy(h)
+
+
+@pytest.mark.parametrize("variant", ["exact_z", "bz0", "bz_neg", "fine_bins", "low_pt"])
+def test_variants(B, variant):
+    spec = dataclasses.replace(W.CONFIGS["central"], n_hyp=4, number=11)
+    over = {}
+    if variant == "exact_z":
+        spec = dataclasses.replace(spec, exact_z=True)         # tracklet z not on pad-row centres
+    elif variant == "bz0":
+        spec = dataclasses.replace(spec, bz=0.0)               # straight lines
+    elif variant == "bz_neg":
+        spec = dataclasses.replace(spec, bz=-0.5)
+    elif variant == "fine_bins":
+        over = dict(ybin_width=0.1)
+    elif variant == "low_pt":
+        spec = dataclasses.replace(spec, pt_spectrum="exp")    # sector crossings, tracks that curl up
+    d = W.generate(spec); cfg = dict(W.matcher_config(spec), **over)
+    want = O.match(cfg, d); got = run_gpu(B, cfg, d)
+    assert_parity(P.compare(got, want), want)
+
+
+def test_host_entry_points_equal_device_entry_points(B):
+    spec = W.CONFIGS["central8"]; d = W.generate(spec); cfg = W.matcher_config(spec)
+    dev_out = run_gpu(B, cfg, d)
+    h = B.trd_create(cfg)
+    try:
+        B.trd_load_tracklets_host(h, d["tl_y"], d["tl_z"], d["tl_dydx"], d["tl_chamber"])
+        out = B.trd_match_host(h, d)
+    finally:
+        B.trd_destroy(h)
+    for k in ("idx", "par", "cov", "x", "sector", "chi2", "n_matched", "n_evals"):
+        np.testing.assert_array_equal(out[k], dev_out[k])
+
+
+def test_quality_trend_of_the_paper(B):
+    """purity ~1 at low density and falling with density (config 1 >= 2 >= 4)."""
+    pur = []
+    for name in ("tiny", "central", "pileup"):
+        spec = W.CONFIGS[name]; d = W.generate(spec)
+        got = run_gpu(B, W.matcher_config(spec), d)
+        q = W.efficiency_purity(got["idx"].T, d)
+        pur.append(q["purity"])
+        assert q["efficiency"] > 0.9
+    assert pur[0] >= pur[1] >= pur[2] and pur[0] > 0.99
