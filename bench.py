@@ -1,0 +1,327 @@
+#!/usr/bin/env python
+"""bench.py -- ITS-TPC tracks matched per second through the 6 TRD layers (BASELINE.json `metric`).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload timeframe]
+
+One "step" is one pass of the whole hot path over one synthetic time frame (BASELINE.json configs[4]:
+2,000,000 tracks, ~18.8M tracklets, nHyp = 4, 3 sigma road): ONE trd_load_tracklets (key, radix sort,
+gather, bin table) + FOUR trd_match calls of 500k tracks.  `value` is timed with inputs resident in HBM;
+`e2e` goes through the *_host entry points of the C ABI with pinned host buffers, copies inside the timed
+region.  N > 1 (torchrun): every rank runs the whole path on its own time frame, no data-path collective
+(weak scaling); barrier + max over ranks.  `--impl reference` times the oracle (oracle/, double precision,
+OpenMP over tracks) on the host cores on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "ITS-TPC tracks matched/sec through 6 TRD layers"
+UNIT = "tracks/s"
+
+# Algorithmic flops per unit, counted from the formulas of DESIGN.md "Arithmetic" (= SURVEY.md 8(d).3):
+# FMA = 2, add/mul/compare = 1, div/sqrt = 1.  Units per launch come from the oracle's counters.
+FLOP = dict(n_prop=180, n_rot=60, n_road=25, n_cand=12, n_upd=110)
+BYTES_TRACK_IN = 88       # 5 + 15 floats, x, sector
+BYTES_TRACK_OUT = 124     # 6 indices, 5 + 15 floats, x, sector, chi2, n_matched, n_cand_evals
+BYTES_PER_CAND = 16       # one (y, z, dy/dx, position) store entry per candidate evaluation
+ORACLE_SAMPLE_TRACKS = 20_000
+
+
+def fp32_peak_tflops(sm_count: int, sm_mhz: float) -> float:
+    """Plain FP32 ALUs: SMs x 128 lanes x 2 flop (FMA) x clock (B200_PROFILING.md: 148 SMs, 1965 MHz)."""
+    return sm_count * 128 * 2 * sm_mhz * 1e6 / 1e12
+
+
+def measured_peaks() -> dict:
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            p = json.load(f)
+        return dict(hbm_gbs=float(p["hbm_gbs"]), sm_max_mhz=float(p.get("sm_max_mhz", 1965.0)), source="measured")
+    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons with NVML while the timed region runs."""
+    REASONS = {0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+               0x80: "hw_power_brake_slowdown", 0x2: "applications_clocks_setting", 0x10: "sync_boost"}
+
+    def __init__(self, uuid: str, index: int, period: float = 0.01):
+        self.period, self.samples, self.mask, self.max_mhz = period, [], 0, None
+        self._stop = threading.Event()
+        self._thread = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            try:
+                self.dev = pynvml.nvmlDeviceGetHandleByUUID(uuid if uuid.startswith("GPU-") else "GPU-" + uuid)
+            except Exception:
+                self.dev = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.dev, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self.nv = None
+
+    def _run(self):
+        while not self._stop.is_set():
+            try:
+                self.samples.append(float(self.nv.nvmlDeviceGetClockInfo(self.dev, self.nv.NVML_CLOCK_SM)))
+                self.mask |= int(self.nv.nvmlDeviceGetCurrentClocksEventReasons(self.dev))
+            except Exception:
+                pass
+            self._stop.wait(self.period)
+
+    def __enter__(self):
+        if self.nv is not None:
+            self._thread = threading.Thread(target=self._run, daemon=True)
+            self._thread.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        if self._thread:
+            self._thread.join()
+
+    def summary(self) -> dict:
+        if not self.samples:
+            return dict(sm_mhz=None, sm_max_mhz=self.max_mhz, reasons=["unavailable"])
+        return dict(sm_mhz=float(np.median(self.samples)), sm_max_mhz=self.max_mhz, n_samples=len(self.samples),
+                    reasons=[name for bit, name in self.REASONS.items() if self.mask & bit])
+
+
+def load_units(spec, n_batches):
+    """Oracle operation counters per trd_match launch of the timeframe config (tests/golden/units_timeframe.json,
+    written by tests/golden/make_units.py from the oracle alone)."""
+    path = os.path.join(ROOT, "tests", "golden", "units_timeframe.json")
+    if spec.name != "timeframe" or not os.path.exists(path):
+        return None
+    with open(path) as f:
+        u = json.load(f)
+    if u["n_tracks"] != spec.n_tracks or len(u["batches"]) != n_batches:
+        return None
+    return u["batches"]
+
+
+def oracle_sample(cfg, data, n_sample, n_threads=0):
+    """The oracle, as it stands, on the first n_sample tracks against ALL tracklets."""
+    from oracle import oracle as O
+    r = O.match(cfg, data, lo=0, hi=n_sample, n_threads=n_threads)
+    cores = O.max_threads() if n_threads == 0 else n_threads
+    return r, cores
+
+
+def run_reference(args, spec, cfg):
+    from paper_2003_03174_b200 import dist as D, workloads as W
+    rank, world, _ = D.env_rank()
+    if rank != 0:
+        return
+    data = W.generate(spec)
+    n_sample = min(ORACLE_SAMPLE_TRACKS, spec.n_tracks)
+    for _ in range(args.warmup):
+        oracle_sample(cfg, data, n_sample)
+    t0 = time.perf_counter()
+    secs = []
+    for _ in range(args.steps):
+        r, cores = oracle_sample(cfg, data, n_sample)
+        secs.append(r["seconds"])
+    wall = time.perf_counter() - t0
+    # whole-job estimate: one index build + the matching of all tracks at the sample's rate
+    idx_s = float(np.mean([s["index"] for s in secs])); match_s = float(np.mean([s["match"] for s in secs]))
+    full_s = idx_s + match_s * spec.n_tracks / n_sample
+    value = spec.n_tracks / full_s
+    sample = (f"{n_sample} of {spec.n_tracks} tracks against all {data['tl_y'].shape[0]} tracklets per step; "
+              f"value = n_tracks / (index build {idx_s:.2f} s + match {match_s:.2f} s x {spec.n_tracks / n_sample:.0f})")
+    line = dict(impl="reference", metric=METRIC, value=value, unit=UNIT, n_gpus=args.gpus, steps=args.steps,
+                warmup=args.warmup, ms_per_step=1e3 * wall / max(args.steps, 1), higher_is_better=True, scaling="weak",
+                vs_baseline=None, dtype="f64", data="synthetic",
+                config=dict(workload=spec.name, n_tracks=spec.n_tracks, n_tracklets=int(data["tl_y"].shape[0]),
+                            n_hyp=spec.n_hyp, n_sigma_road=spec.n_sigma_road),
+                cpu_baseline=dict(value=value, unit=UNIT, cores=cores, kind="oracle", sample=sample),
+                e2e=dict(value=value, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0), gpu_launches=0)
+    print(json.dumps(line), flush=True)
+
+
+def run_ours(args, spec, cfg):
+    import torch
+    from paper_2003_03174_b200 import binding as B, build as Bd, dist as D, workloads as W
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the TRD matcher has no CPU fallback")
+    rank, world, local = D.env_rank()
+    torch.cuda.set_device(local)
+    device = torch.device("cuda", local)
+    D.init("nccl")
+    if rank == 0:
+        Bd.build()
+    D.barrier()
+    data = W.generate(spec)                     # every rank: its own (identically generated) time frame
+    n, n_tl = spec.n_tracks, int(data["tl_y"].shape[0])
+    batch = spec.batch or n
+    bounds = [(lo, min(n, lo + batch)) for lo in range(0, n, batch)]
+    dev = B.to_device(data, device)
+    tracks = [dict(par=dev["par"][:, lo:hi].contiguous(), cov=dev["cov"][:, lo:hi].contiguous(),
+                   x=dev["x"][lo:hi].contiguous(), sector=dev["sector"][lo:hi].contiguous()) for lo, hi in bounds]
+    outs = [B.alloc_tracks_out(hi - lo, device) for lo, hi in bounds]
+    tl = (dev["tl_y"], dev["tl_z"], dev["tl_dydx"], dev["tl_chamber"])
+    h = B.trd_create(cfg)
+    stream = torch.cuda.current_stream()
+
+    def step(ev=None):
+        if ev is not None:
+            ev.append(torch.cuda.Event(enable_timing=True)); ev[-1].record(stream)
+        B.trd_load_tracklets(h, *tl, stream=stream)
+        for t, o in zip(tracks, outs):
+            if ev is not None:
+                ev.append(torch.cuda.Event(enable_timing=True)); ev[-1].record(stream)
+            B.trd_match(h, t, o, stream=stream)
+        if ev is not None:
+            ev.append(torch.cuda.Event(enable_timing=True)); ev[-1].record(stream)
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize(); D.barrier()
+    launches0 = B.trd_kernel_launches(h)
+    events = []
+    with ClockSampler(str(getattr(torch.cuda.get_device_properties(local), "uuid", "")), local) as clk:
+        t_start = torch.cuda.Event(enable_timing=True); t_end = torch.cuda.Event(enable_timing=True)
+        t_start.record(stream)
+        for _ in range(args.steps):
+            ev = []; step(ev); events.append(ev)
+        t_end.record(stream)
+        torch.cuda.synchronize()
+    D.barrier()
+    launches = B.trd_kernel_launches(h) - launches0
+    total_ms = D.max_over_ranks(t_start.elapsed_time(t_end), device)
+    ms_per_step = total_ms / args.steps
+    value = world * n / (ms_per_step * 1e-3)
+    nb = len(bounds)
+    load_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in events]))
+    match_ms = np.array([[e[1 + k].elapsed_time(e[2 + k]) for k in range(nb)] for e in events])   # steps x batches
+    n_evals = int(sum(int(o["n_evals"].sum().item()) for o in outs))
+    n_ge2 = int(sum(int((o["n_matched"] >= 2).sum().item()) for o in outs))
+
+    # ---- end to end through the host entry points (pinned host buffers, copies inside the timed region)
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy()   # noqa: E731
+    h_tl = [pin(data[k]) for k in ("tl_y", "tl_z", "tl_dydx", "tl_chamber")]
+    h_tracks = [dict(par=pin(data["par"][:, lo:hi]), cov=pin(data["cov"][:, lo:hi]), x=pin(data["x"][lo:hi]),
+                     sector=pin(data["sector"][lo:hi])) for lo, hi in bounds]
+    h_outs = [B.alloc_tracks_out_host(hi - lo, pinned=True) for lo, hi in bounds]
+
+    def step_host():
+        B.trd_load_tracklets_host(h, *h_tl, stream=stream)
+        for t, o in zip(h_tracks, h_outs):
+            B.trd_match_host(h, t, o, stream=stream)
+
+    for _ in range(2):
+        step_host()
+    torch.cuda.synchronize(); D.barrier()
+    e2e_steps = max(1, min(args.steps, 5))
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        step_host()
+    torch.cuda.synchronize()
+    e2e_s = D.max_over_ranks(time.perf_counter() - t0, device) / e2e_steps
+    D.barrier()
+    for o, ho in zip(outs, h_outs):               # the two entry points must agree bit for bit
+        assert np.array_equal(o["idx"].cpu().numpy(), ho["idx"]) and np.array_equal(o["chi2"].cpu().numpy(), ho["chi2"])
+    h2d = 16 * n_tl + BYTES_TRACK_IN * n
+    d2h = BYTES_TRACK_OUT * n
+    info = B.trd_get_index_info(h)
+    B.trd_destroy(h)
+
+    if rank != 0:
+        D.shutdown()
+        return
+    # ---- roofline of the dominant kernel: match_kernel (4 launches per step) vs the load
+    peaks = measured_peaks()
+    props = torch.cuda.get_device_properties(local)
+    clocks = clk.summary()
+    units = load_units(spec, nb)
+    match_avg_ms = float(match_ms.mean())
+    peak_tf = fp32_peak_tflops(props.multi_processor_count, peaks["sm_max_mhz"])
+    if units is not None:
+        flops = float(np.mean([sum(FLOP[k] * u[k] for k in FLOP) for u in units]))
+        cand = float(np.mean([u["n_cand"] for u in units]))
+        units_src = "tests/golden/units_timeframe.json (oracle counters per 500k-track launch)"
+    else:                                          # other workloads: count what the GPU itself reported
+        flops, cand, units_src = None, n_evals / nb, "n_cand from the kernel's own counter; flops not frozen for this workload"
+    bytes_alg = (BYTES_TRACK_IN + BYTES_TRACK_OUT) * (n / nb) + min(cand, n_tl) * BYTES_PER_CAND
+    t_hbm = bytes_alg / (peaks["hbm_gbs"] * 1e9)
+    t_alu = (flops / (peak_tf * 1e12)) if flops else 0.0
+    if t_alu >= t_hbm:
+        ach = flops / (match_avg_ms * 1e-3) / 1e12
+        roof = dict(bound="alu", achieved=ach, peak=peak_tf, unit="TFLOP/s", frac=ach / peak_tf, traffic=None)
+    else:
+        ach = bytes_alg / (match_avg_ms * 1e-3) / 1e9
+        roof = dict(bound="hbm", achieved=ach, peak=peaks["hbm_gbs"], unit="GB/s", frac=ach / peaks["hbm_gbs"], traffic=None)
+    roof.update(kernel="match_kernel<4>" if spec.n_hyp in (3, 4) else f"match_kernel (n_hyp={spec.n_hyp})",
+                launch_ms=match_avg_ms, launches_per_step=nb, share_of_step=nb * match_avg_ms / ms_per_step,
+                algorithmic_flops_per_launch=flops, algorithmic_bytes_per_launch=bytes_alg,
+                roofline_ms_per_launch=1e3 * max(t_alu, t_hbm), hbm_view_gbs=bytes_alg / (match_avg_ms * 1e-3) / 1e9,
+                peak_source=f"HBM {peaks['source']} (MEASURED_PEAKS.json); FP32 = {props.multi_processor_count} SMs x 128 x 2 x "
+                            f"{peaks['sm_max_mhz']:.0f} MHz", units=units_src,
+                load_tracklets_ms=load_ms, load_algorithmic_gbs=n_tl * (52 + 20 * info["n_passes"]) / (load_ms * 1e-3) / 1e9)
+    prof = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(prof):
+        with open(prof) as f:
+            roof["traffic"] = json.load(f).get("match_kernel_dram_bytes_per_launch")
+
+    line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=max(args.warmup, 3),
+                ms_per_step=ms_per_step, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32",
+                data="synthetic",
+                config=dict(workload=spec.name, n_tracks=n, n_tracklets=n_tl, n_hyp=spec.n_hyp, n_sigma_road=spec.n_sigma_road,
+                            batch=batch, step="1 trd_load_tracklets + %d trd_match" % nb,
+                            l2="inputs larger than L2 (%.0f MB tracklets + %.0f MB tracks per step)" % (16e-6 * n_tl, 88e-6 * n),
+                            parallelism=f"{world} x independent time frames, no collective"),
+                cand_evals_per_s=world * n_evals / (ms_per_step * 1e-3), n_cand_evals=n_evals,
+                frac_tracks_ge2_tracklets=n_ge2 / n, index=dict(n_ybins=info["n_ybins"], n_zrows=info["n_zrows"],
+                                                                ybin_width_cm=info["ybin_width"], radix_passes=info["n_passes"]),
+                clocks=clocks, gpu_launches=int(launches),
+                e2e=dict(value=world * n / e2e_s, unit=UNIT, h2d_bytes_per_step=int(h2d), d2h_bytes_per_step=int(d2h),
+                         ms_per_step=1e3 * e2e_s, steps=e2e_steps),
+                roofline=roof)
+    if world == 1 and not args.no_cpu_baseline:
+        n_sample = min(ORACLE_SAMPLE_TRACKS, n)
+        r, cores = oracle_sample(cfg, data, n_sample)
+        full_s = r["seconds"]["index"] + r["seconds"]["match"] * n / n_sample
+        line["cpu_baseline"] = dict(
+            value=n / full_s, unit=UNIT, cores=cores, kind="oracle",
+            sample=(f"first {n_sample} of {n} tracks against all {n_tl} tracklets: index build {r['seconds']['index']:.2f} s + "
+                    f"match {r['seconds']['match']:.2f} s; value = n_tracks / (index + match x {n / n_sample:.0f})"))
+    print(json.dumps(line), flush=True)
+    D.shutdown()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="timeframe")
+    ap.add_argument("--tracks", type=int, default=0, help="scale the workload to this many tracks (debugging)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    from paper_2003_03174_b200 import workloads as W
+    spec = W.CONFIGS[args.workload]
+    if args.tracks:
+        spec = W.scaled(spec, args.tracks)
+    cfg = W.matcher_config(spec)
+    if args.impl == "reference":
+        run_reference(args, spec, cfg)
+    else:
+        run_ours(args, spec, cfg)
+
+
+if __name__ == "__main__":
+    main()
