@@ -69,6 +69,11 @@ typedef struct trd_config {
     double chi2_penalty;             /* score added for a layer without tracklet (15) */
     double max_snp;                  /* a hypothesis dies at |sin(phi)| >= max_snp (0.95) */
     double ybin_width;               /* local-y bin width of the tracklet index; 0 = chosen per load */
+    int32_t track_binning;           /* trd_match bins the tracks of a batch by predicted (sector, z row, y)
+                                        before matching, for cache locality: 0 = when it pays (large batch
+                                        against a large index), 1 = always, -1 = never.  Results do not
+                                        depend on it. */
+    int32_t reserved_;               /* 0 */
 } trd_config;
 
 /* Input tracks of one batch: device pointers, each of length n_tracks. */

@@ -34,7 +34,8 @@ class TrdConfig(C.Structure):
                 ("z_max", C.c_double), ("pad_length", C.c_double), ("bz_tesla", C.c_double),
                 ("sigma_y", C.c_double), ("sigma_z", C.c_double), ("sigma_dydx", C.c_double),
                 ("n_sigma_road", C.c_double), ("n_sigma_angle", C.c_double), ("chi2_cut", C.c_double),
-                ("chi2_penalty", C.c_double), ("max_snp", C.c_double), ("ybin_width", C.c_double)]
+                ("chi2_penalty", C.c_double), ("max_snp", C.c_double), ("ybin_width", C.c_double),
+                ("track_binning", C.c_int32), ("reserved_", C.c_int32)]
 
 
 class TrdTracksIn(C.Structure):
@@ -105,6 +106,7 @@ def make_config(cfg: dict) -> TrdConfig:
               "n_sigma_angle", "chi2_cut", "chi2_penalty", "max_snp"):
         setattr(c, k, float(cfg[k]))
     c.ybin_width = float(cfg.get("ybin_width", 0.0))
+    c.track_binning = int(cfg.get("track_binning", 0))
     return c
 
 

@@ -69,6 +69,7 @@ const char* check_config(const trd_config& c) {
     if (!(c.chi2_cut > 0.0) || !(c.chi2_penalty >= 0.0)) return "chi2_cut / chi2_penalty out of range";
     if (!(c.max_snp > 0.0) || !(c.max_snp < 1.0)) return "max_snp must be in (0, 1)";
     if (!(c.ybin_width >= 0.0)) return "ybin_width must be >= 0";
+    if (c.track_binning < -1 || c.track_binning > 1) return "track_binning must be -1, 0 or 1";
     return nullptr;
 }
 
@@ -121,6 +122,14 @@ void trd_destroy(trd_handle* h) {
     release(h->stage_tl);
     release(h->stage_in);
     release(h->stage_out);
+    release(h->trk_rec);
+    release(h->trk_out);
+    for (int s = 0; s < 2; ++s) {
+        release(h->trk_key[s]);
+        release(h->trk_val[s]);
+    }
+    release(h->trk_hist);
+    release(h->trk_tot);
     delete h;
 }
 
@@ -254,8 +263,9 @@ const char* trd_last_error(const trd_handle* h) { return h ? h->err.c_str() : "N
 int64_t trd_device_bytes(const trd_handle* h) {
     if (!h) return 0;
     size_t t = h->store.bytes + h->tile_hist.bytes + h->digit_tot.bytes + h->bin_first.bytes + h->stage_tl.bytes +
-               h->stage_in.bytes + h->stage_out.bytes;
-    for (int s = 0; s < 2; ++s) t += h->key[s].bytes + h->val[s].bytes;
+               h->stage_in.bytes + h->stage_out.bytes + h->trk_rec.bytes + h->trk_out.bytes + h->trk_hist.bytes +
+               h->trk_tot.bytes;
+    for (int s = 0; s < 2; ++s) t += h->key[s].bytes + h->val[s].bytes + h->trk_key[s].bytes + h->trk_val[s].bytes;
     return (int64_t)t;
 }
 

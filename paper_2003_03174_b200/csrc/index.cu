@@ -211,6 +211,32 @@ cudaError_t reserve(Buffer& b, size_t bytes, cudaStream_t stream) {
     return cudaSuccess;
 }
 
+int radix_tiles(int64_t n) { return (int)((n + kTile - 1) / kTile); }
+
+// stable LSD radix sort of (key, position) pairs, 8 bits per pass; positions start as 0..n-1.
+// key0/val0 and key1/val1 ping-pong; *side tells which pair holds the result.
+cudaError_t radix_sort_pairs(uint32_t* key0, uint32_t* key1, uint32_t* val0, uint32_t* val1, uint32_t* tile_hist,
+                             uint32_t* digit_tot, int64_t n, int n_passes, cudaStream_t stream, int* side_out,
+                             int64_t* launches) {
+    const int n_tiles = radix_tiles(n);
+    uint32_t* key[2] = {key0, key1};
+    uint32_t* val[2] = {val0, val1};
+    int side = 0;
+    for (int p = 0; p < n_passes; ++p) {
+        const int sh = p * kRadixBits;
+        const uint32_t* kin = key[side];
+        const uint32_t* vin = (p == 0) ? nullptr : val[side];
+        radix_hist<<<n_tiles, kSortThreads, 0, stream>>>(kin, tile_hist, n, n_tiles, sh);
+        radix_rowscan<<<kRadix, kSortThreads, 0, stream>>>(tile_hist, digit_tot, n_tiles);
+        radix_scatter<<<n_tiles, kSortThreads, 0, stream>>>(kin, vin, key[side ^ 1], val[side ^ 1], tile_hist, digit_tot, n,
+                                                           n_tiles, sh);
+        *launches += 3;
+        side ^= 1;
+    }
+    *side_out = side;
+    return cudaGetLastError();
+}
+
 cudaError_t build_index(trd_handle* h, const float* d_y, const float* d_z, const float* d_dydx,
                         const int32_t* d_chamber, int64_t n, cudaStream_t stream) {
     const trd_config& c = h->cfg;
@@ -263,18 +289,8 @@ cudaError_t build_index(trd_handle* h, const float* d_y, const float* d_z, const
     tracklet_key<<<n_blk, 256, 0, stream>>>(d_y, d_z, d_chamber, (uint32_t*)h->key[0].p, n, g);
     h->launches++;
     int side = 0;
-    for (int p = 0; p < h->n_passes; ++p) {
-        const int sh = p * kRadixBits;
-        const uint32_t* kin = (const uint32_t*)h->key[side].p;
-        const uint32_t* vin = (p == 0) ? nullptr : (const uint32_t*)h->val[side].p;
-        radix_hist<<<n_tiles, kSortThreads, 0, stream>>>(kin, (uint32_t*)h->tile_hist.p, n, n_tiles, sh);
-        radix_rowscan<<<kRadix, kSortThreads, 0, stream>>>((uint32_t*)h->tile_hist.p, (uint32_t*)h->digit_tot.p, n_tiles);
-        radix_scatter<<<n_tiles, kSortThreads, 0, stream>>>(kin, vin, (uint32_t*)h->key[side ^ 1].p,
-                                                           (uint32_t*)h->val[side ^ 1].p, (const uint32_t*)h->tile_hist.p,
-                                                           (const uint32_t*)h->digit_tot.p, n, n_tiles, sh);
-        h->launches += 3;
-        side ^= 1;
-    }
+    TRD_TRY(radix_sort_pairs((uint32_t*)h->key[0].p, (uint32_t*)h->key[1].p, (uint32_t*)h->val[0].p, (uint32_t*)h->val[1].p,
+                             (uint32_t*)h->tile_hist.p, (uint32_t*)h->digit_tot.p, n, h->n_passes, stream, &side, &h->launches));
     h->sorted_side = side;
     gather_store<<<n_blk, 256, 0, stream>>>((const uint32_t*)h->val[side].p, d_y, d_z, d_dydx, (float4*)h->store.p, n);
     bin_first_kernel<<<n_blk, 256, 0, stream>>>((const uint32_t*)h->key[side].p, (int32_t*)h->bin_first.p, n, g.n_bins);

@@ -1,0 +1,119 @@
+// tracks.cu -- track binning around the match kernel ("track pre-binning").
+//
+// Tracks arrive in arbitrary order, so neighbouring sub-warps of the match kernel would touch
+// unrelated bins of the tracklet index and re-read it from HBM many times.  For large batches
+// trd_match therefore (1) packs every track into one 96-byte record and computes a locality key
+// (sector, z row, coarse y of the straight-line prediction at the middle TRD layer), (2) radix-sorts
+// the keys (index.cu), (3) runs the match kernel over the sorted permutation, gathering whole
+// records and scattering whole 128-byte result records, (4) unpacks the results to the caller's
+// SoA arrays.  The key only decides the processing order; no result depends on it.
+#include "trd_internal.cuh"
+
+namespace trd {
+
+namespace {
+
+constexpr int kThreads = 128;
+constexpr int kYBits = 4;                      // 16 coarse y bins per (sector, z row)
+
+// SoA -> records through shared memory so that both sides are coalesced
+__global__ void __launch_bounds__(kThreads) pack_kernel(const trd_tracks_in in, int64_t n, float* __restrict__ rec,
+                                                        uint32_t* __restrict__ key, IndexGeom g, float x_mid, float edge_mid,
+                                                        int nz) {
+    __shared__ float sm[kThreads][kRecIn + 1];
+    const int64_t base = (int64_t)blockIdx.x * kThreads;
+    const int64_t i = base + threadIdx.x;
+    if (i < n) {
+        float* r = sm[threadIdx.x];
+#pragma unroll
+        for (int k = 0; k < 5; ++k) r[k] = in.par[k][i];
+#pragma unroll
+        for (int k = 0; k < 15; ++k) r[5 + k] = in.cov[k][i];
+        const float x = in.x[i];
+        const int sector = in.sector[i];
+        r[20] = x;
+        r[21] = __int_as_float(sector);
+        r[22] = 0.0f;
+        r[23] = 0.0f;
+        // locality key from the straight-line prediction at x_mid
+        const float s = fminf(fmaxf(r[2], -0.99f), 0.99f);
+        const float inv_c = rsqrtf((1.0f - s) * (1.0f + s));
+        const float dx = x_mid - x;
+        float yp = fmaf(dx, s * inv_c, r[0]);
+        const float zp = fmaf(dx, r[3] * inv_c, r[1]);
+        int sec = sector;
+        if (yp > edge_mid) { sec += 1; yp -= 2.0f * edge_mid; }
+        if (yp < -edge_mid) { sec -= 1; yp += 2.0f * edge_mid; }
+        sec = ((sec % g.n_sectors) + g.n_sectors) % g.n_sectors;
+        float fy = floorf((yp + edge_mid) / (2.0f * edge_mid) * (float)(1 << kYBits));
+        fy = fminf(fmaxf(fy, 0.0f), (float)((1 << kYBits) - 1));
+        const int zr = isfinite(zp) ? zrow_of(g, zp) : 0;
+        key[i] = (((uint32_t)sec * (uint32_t)nz + (uint32_t)zr) << kYBits) + (uint32_t)(isfinite(fy) ? (int)fy : 0);
+    }
+    __syncthreads();
+    const int64_t n_here = min((int64_t)kThreads, n - base);
+    const int64_t n_f4 = n_here * (kRecIn / 4);
+    float4* dst = reinterpret_cast<float4*>(rec + base * kRecIn);
+    for (int64_t j = threadIdx.x; j < n_f4; j += kThreads) {
+        const int f = (int)j * 4, t = f / kRecIn, w = f % kRecIn;
+        dst[j] = make_float4(sm[t][w], sm[t][w + 1], sm[t][w + 2], sm[t][w + 3]);
+    }
+}
+
+// result records (caller's order) -> SoA
+__global__ void __launch_bounds__(kThreads) unpack_kernel(const float* __restrict__ rec, const trd_tracks_out out, int64_t n,
+                                                          int n_layers) {
+    __shared__ float sm[kThreads][kRecOut + 1];
+    const int64_t base = (int64_t)blockIdx.x * kThreads;
+    const int64_t n_here = min((int64_t)kThreads, n - base);
+    const int64_t n_f4 = n_here * (kRecOut / 4);
+    const float4* src = reinterpret_cast<const float4*>(rec + base * kRecOut);
+    for (int64_t j = threadIdx.x; j < n_f4; j += kThreads) {
+        const float4 v = src[j];
+        const int f = (int)j * 4, t = f / kRecOut, w = f % kRecOut;
+        sm[t][w] = v.x; sm[t][w + 1] = v.y; sm[t][w + 2] = v.z; sm[t][w + 3] = v.w;
+    }
+    __syncthreads();
+    const int64_t i = base + threadIdx.x;
+    if (i >= n) return;
+    const float* r = sm[threadIdx.x];
+#pragma unroll
+    for (int l = 0; l < TRD_MAX_LAYERS; ++l) out.tracklet_idx[l][i] = (l < n_layers) ? __float_as_int(r[l]) : -1;
+#pragma unroll
+    for (int k = 0; k < 5; ++k) out.par[k][i] = r[6 + k];
+#pragma unroll
+    for (int k = 0; k < 15; ++k) out.cov[k][i] = r[11 + k];
+    out.x[i] = r[26];
+    out.sector[i] = __float_as_int(r[27]);
+    out.chi2[i] = r[28];
+    out.n_matched[i] = __float_as_int(r[29]);
+    if (out.n_cand_evals) out.n_cand_evals[i] = __float_as_int(r[30]);
+}
+
+}  // namespace
+
+cudaError_t pack_tracks(trd_handle* h, const trd_tracks_in& in, int64_t n, float* rec, uint32_t* key, int* key_bits,
+                        cudaStream_t stream) {
+    const trd_config& c = h->cfg;
+    const IndexGeom& g = h->mp.g;
+    const int mid = c.n_layers / 2;
+    const float x_mid = (float)c.layer_x[mid];
+    const float edge_mid = (float)(c.layer_x[mid] * tan(M_PI / c.n_sectors));
+    const unsigned grid = (unsigned)((n + kThreads - 1) / kThreads);
+    pack_kernel<<<grid, kThreads, 0, stream>>>(in, n, rec, key, g, x_mid, edge_mid, g.nz);
+    h->launches++;
+    uint64_t n_keys = ((uint64_t)c.n_sectors * g.nz) << kYBits;
+    int bits = 0;
+    while ((1ull << bits) < n_keys) ++bits;
+    *key_bits = bits;
+    return cudaGetLastError();
+}
+
+cudaError_t unpack_tracks(trd_handle* h, const float* rec_out, const trd_tracks_out& out, int64_t n, cudaStream_t stream) {
+    const unsigned grid = (unsigned)((n + kThreads - 1) / kThreads);
+    unpack_kernel<<<grid, kThreads, 0, stream>>>(rec_out, out, n, h->cfg.n_layers);
+    h->launches++;
+    return cudaGetLastError();
+}
+
+}  // namespace trd

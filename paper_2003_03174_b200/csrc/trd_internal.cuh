@@ -78,6 +78,13 @@ struct trd_handle {
     trd::Buffer stage_tl;   // tracklets
     trd::Buffer stage_in;   // tracks in
     trd::Buffer stage_out;  // tracks out
+    // track binning (trd_match on large batches): packed records and the permutation
+    trd::Buffer trk_rec;    // kRecIn floats per track, caller's order
+    trd::Buffer trk_out;    // kRecOut floats per track, caller's order
+    trd::Buffer trk_key[2]; // uint32 bin keys, ping-pong
+    trd::Buffer trk_val[2]; // uint32 track positions, ping-pong
+    trd::Buffer trk_hist;   // [256][n_tiles]
+    trd::Buffer trk_tot;    // [256]
 };
 
 namespace trd {
@@ -87,6 +94,19 @@ cudaError_t build_index(trd_handle* h, const float* d_y, const float* d_z, const
                         const int32_t* d_chamber, int64_t n, cudaStream_t stream);
 cudaError_t launch_match(trd_handle* h, const trd_tracks_in& in, const trd_tracks_out& out, int64_t n,
                          cudaStream_t stream);
+
+// packed track records used when a batch is binned before matching (tracks.cu, match.cu)
+constexpr int kRecIn = 24;    // y z s t c | 15 cov | x | sector bits | 2 pad          (96 bytes)
+constexpr int kRecOut = 32;   // 6 idx | 5 par | 15 cov | x sector chi2 n_matched n_evals | pad   (128 bytes)
+
+int radix_tiles(int64_t n);
+cudaError_t radix_sort_pairs(uint32_t* key0, uint32_t* key1, uint32_t* val0, uint32_t* val1, uint32_t* tile_hist,
+                             uint32_t* digit_tot, int64_t n, int n_passes, cudaStream_t stream, int* side_out,
+                             int64_t* launches);
+// tracks.cu: SoA -> packed records + locality key; packed results -> SoA
+cudaError_t pack_tracks(trd_handle* h, const trd_tracks_in& in, int64_t n, float* rec, uint32_t* key, int* key_bits,
+                        cudaStream_t stream);
+cudaError_t unpack_tracks(trd_handle* h, const float* rec_out, const trd_tracks_out& out, int64_t n, cudaStream_t stream);
 
 // grows b to at least `bytes` (contents lost); synchronises `stream` before freeing
 cudaError_t reserve(Buffer& b, size_t bytes, cudaStream_t stream);

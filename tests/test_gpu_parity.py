@@ -200,3 +200,20 @@ def test_quality_trend_of_the_paper(B):
         pur.append(q["purity"])
         assert q["efficiency"] > 0.9
     assert pur[0] >= pur[1] >= pur[2] and pur[0] > 0.99
+
+
+@pytest.mark.parametrize("name", ["tiny", "central8", "pileup"])
+def test_track_binning_does_not_change_results(B, name):
+    """trd_config.track_binning only changes the processing order (tracks.cu): bit-identical outputs with
+    binning forced on and off, also with in-place outputs and ragged batches."""
+    spec = W.CONFIGS[name]; d = W.generate(spec); cfg = W.matcher_config(spec)
+    off = run_gpu(B, dict(cfg, track_binning=-1), d)
+    on = run_gpu(B, dict(cfg, track_binning=1), d)
+    on_inplace = run_gpu(B, dict(cfg, track_binning=1), d, in_place=True)
+    on_ragged = run_gpu(B, dict(cfg, track_binning=1), d, batch=777)
+    for k in ("idx", "par", "cov", "x", "sector", "chi2", "n_matched", "n_evals"):
+        np.testing.assert_array_equal(on[k], off[k])
+        np.testing.assert_array_equal(on_inplace[k], off[k])
+        np.testing.assert_array_equal(on_ragged[k], off[k])
+    want = O.match(cfg, d)
+    assert_parity(P.compare(on, want), want)
