@@ -136,7 +136,7 @@ void trd_destroy(trd_handle* h) {
 int trd_load_tracklets(trd_handle* h, const float* d_y, const float* d_z, const float* d_dydx,
                        const int32_t* d_chamber, int64_t n, void* stream) {
     if (!h) return TRD_E_ARG;
-    if (n < 0 || n > 0x7fffffff) return fail(h, TRD_E_ARG, "trd_load_tracklets: n out of range");
+    if (n < 0 || n >= (1 << 29) - 1) return fail(h, TRD_E_ARG, "trd_load_tracklets: n out of range (must be < 2^29 - 1)");
     if (n > 0 && (!d_y || !d_z || !d_dydx || !d_chamber)) return fail(h, TRD_E_ARG, "trd_load_tracklets: NULL array");
     const cudaError_t e = trd::build_index(h, d_y, d_z, d_dydx, d_chamber, n, (cudaStream_t)stream);
     if (e != cudaSuccess) return fail_cuda(h, e, "trd_load_tracklets");
@@ -164,7 +164,7 @@ int trd_match(trd_handle* h, const trd_tracks_in* in, const trd_tracks_out* out,
 int trd_load_tracklets_host(trd_handle* h, const float* y, const float* z, const float* dydx,
                             const int32_t* chamber, int64_t n, void* stream) {
     if (!h) return TRD_E_ARG;
-    if (n < 0 || n > 0x7fffffff) return fail(h, TRD_E_ARG, "trd_load_tracklets_host: n out of range");
+    if (n < 0 || n >= (1 << 29) - 1) return fail(h, TRD_E_ARG, "trd_load_tracklets_host: n out of range (must be < 2^29 - 1)");
     if (n > 0 && (!y || !z || !dydx || !chamber)) return fail(h, TRD_E_ARG, "trd_load_tracklets_host: NULL array");
     cudaStream_t st = (cudaStream_t)stream;
     const size_t bytes = (size_t)n * 4;
