@@ -24,12 +24,16 @@ constexpr int kSortWarps = kSortThreads / 32;
 constexpr int kItems = 16;                          // keys per thread and tile
 constexpr int kTile = kSortThreads * kItems;        // 4096 keys per tile
 
+// also packs (y, z, dy/dx, position) into one 16-byte record so that the gather after the sort reads
+// one sector per tracklet instead of three
 __global__ void __launch_bounds__(256) tracklet_key(const float* __restrict__ y, const float* __restrict__ z,
-                                                    const int32_t* __restrict__ chamber, uint32_t* __restrict__ key,
-                                                    int64_t n, IndexGeom g) {
+                                                    const float* __restrict__ dydx, const int32_t* __restrict__ chamber,
+                                                    uint32_t* __restrict__ key, float4* __restrict__ packed, int64_t n,
+                                                    IndexGeom g) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     const float yy = y[i], zz = z[i];
+    packed[i] = make_float4(yy, zz, dydx[i], __uint_as_float((uint32_t)i));
     const int ch = chamber[i];
     uint32_t k = g.n_bins;                          // unusable: behind every bin
     if (ch >= 0 && ch < g.n_chambers && isfinite(yy) && isfinite(zz)) {
@@ -162,13 +166,11 @@ __global__ void __launch_bounds__(kSortThreads) radix_scatter(const uint32_t* __
     }
 }
 
-__global__ void __launch_bounds__(256) gather_store(const uint32_t* __restrict__ pos, const float* __restrict__ y,
-                                                    const float* __restrict__ z, const float* __restrict__ dydx,
+__global__ void __launch_bounds__(256) gather_store(const uint32_t* __restrict__ pos, const float4* __restrict__ packed,
                                                     float4* __restrict__ store, int64_t n) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
-    const uint32_t j = pos[i];
-    store[i] = make_float4(y[j], z[j], dydx[j], __uint_as_float(j));
+    store[i] = __ldg(packed + pos[i]);
 }
 
 // bin_first[b] = first sorted position whose key is >= b, for b = 0..n_bins
@@ -278,6 +280,7 @@ cudaError_t build_index(trd_handle* h, const float* d_y, const float* d_z, const
     }
     const int n_tiles = (int)((n + kTile - 1) / kTile);
     TRD_TRY(reserve(h->store, (size_t)n * sizeof(float4), stream));
+    TRD_TRY(reserve(h->packed, (size_t)n * sizeof(float4), stream));
     for (int s = 0; s < 2; ++s) {
         TRD_TRY(reserve(h->key[s], (size_t)n * sizeof(uint32_t), stream));
         TRD_TRY(reserve(h->val[s], (size_t)n * sizeof(uint32_t), stream));
@@ -286,13 +289,13 @@ cudaError_t build_index(trd_handle* h, const float* d_y, const float* d_z, const
     TRD_TRY(reserve(h->digit_tot, kRadix * sizeof(uint32_t), stream));
 
     const unsigned n_blk = (unsigned)((n + 255) / 256);
-    tracklet_key<<<n_blk, 256, 0, stream>>>(d_y, d_z, d_chamber, (uint32_t*)h->key[0].p, n, g);
+    tracklet_key<<<n_blk, 256, 0, stream>>>(d_y, d_z, d_dydx, d_chamber, (uint32_t*)h->key[0].p, (float4*)h->packed.p, n, g);
     h->launches++;
     int side = 0;
     TRD_TRY(radix_sort_pairs((uint32_t*)h->key[0].p, (uint32_t*)h->key[1].p, (uint32_t*)h->val[0].p, (uint32_t*)h->val[1].p,
                              (uint32_t*)h->tile_hist.p, (uint32_t*)h->digit_tot.p, n, h->n_passes, stream, &side, &h->launches));
     h->sorted_side = side;
-    gather_store<<<n_blk, 256, 0, stream>>>((const uint32_t*)h->val[side].p, d_y, d_z, d_dydx, (float4*)h->store.p, n);
+    gather_store<<<n_blk, 256, 0, stream>>>((const uint32_t*)h->val[side].p, (const float4*)h->packed.p, (float4*)h->store.p, n);
     bin_first_kernel<<<n_blk, 256, 0, stream>>>((const uint32_t*)h->key[side].p, (int32_t*)h->bin_first.p, n, g.n_bins);
     h->launches += 2;
     TRD_TRY(cudaGetLastError());

@@ -68,6 +68,7 @@ struct trd_handle {
     std::string err;
     // device buffers owned by the handle
     trd::Buffer store;      // float4 per sorted tracklet: y, z, dy/dx, original position (bits)
+    trd::Buffer packed;     // float4 per tracklet in the caller's order (gather source)
     trd::Buffer key[2];     // uint32 keys, ping-pong
     trd::Buffer val[2];     // uint32 original positions, ping-pong
     trd::Buffer tile_hist;  // [256][n_tiles] digit counts per tile
