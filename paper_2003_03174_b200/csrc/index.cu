@@ -104,7 +104,8 @@ __global__ void __launch_bounds__(kSortThreads) radix_rowscan(uint32_t* __restri
 }
 
 // stable scatter of one tile.  Order inside a tile is (warp, round, lane): warp w owns the
-// contiguous keys [w * kItems * 32, (w + 1) * kItems * 32) of the tile.
+// contiguous keys [w * kItems * 32, (w + 1) * kItems * 32) of the tile.  The tile is first reordered by
+// digit in shared memory so that the global writes go out as contiguous runs per digit.
 __global__ void __launch_bounds__(kSortThreads) radix_scatter(const uint32_t* __restrict__ key_in,
                                                               const uint32_t* __restrict__ val_in,
                                                               uint32_t* __restrict__ key_out, uint32_t* __restrict__ val_out,
@@ -112,7 +113,9 @@ __global__ void __launch_bounds__(kSortThreads) radix_scatter(const uint32_t* __
                                                               const uint32_t* __restrict__ digit_tot, int64_t n, int n_tiles,
                                                               int shift) {
     __shared__ uint32_t warp_cnt[kSortWarps][kRadix];
-    __shared__ uint32_t digit_base[kRadix];
+    __shared__ uint32_t digit_base[kRadix];    // global position of the tile's first key with digit d
+    __shared__ uint32_t tile_off[kRadix];      // position inside the reordered tile of its first key with digit d
+    __shared__ uint32_t s_key[kTile], s_val[kTile];
     __shared__ uint32_t warp_sums[32];
     __shared__ uint32_t total;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -123,7 +126,8 @@ __global__ void __launch_bounds__(kSortThreads) radix_scatter(const uint32_t* __
     const uint32_t ex = block_exclusive_scan(digit_tot[threadIdx.x], warp_sums, &total);   // syncs
     digit_base[threadIdx.x] = ex + hist[(size_t)threadIdx.x * n_tiles + blockIdx.x];
 
-    const int64_t base = (int64_t)blockIdx.x * kTile + (int64_t)warp * (kItems * 32);
+    const int64_t tile_base = (int64_t)blockIdx.x * kTile;
+    const int64_t base = tile_base + (int64_t)warp * (kItems * 32);
     uint32_t k[kItems], v[kItems], rank[kItems];
 #pragma unroll
     for (int r = 0; r < kItems; ++r) {
@@ -136,7 +140,14 @@ __global__ void __launch_bounds__(kSortThreads) radix_scatter(const uint32_t* __
     for (int r = 0; r < kItems; ++r) {
         const bool ok = base + r * 32 + lane < n;
         const uint32_t d = (k[r] >> shift) & (kRadix - 1);
-        const uint32_t peers = __match_any_sync(0xffffffffu, ok ? d : (uint32_t)kRadix);
+        // lanes holding the same digit: one ballot per digit bit (fixed cost, unlike MATCH.ANY whose
+        // latency grows with the number of distinct values)
+        uint32_t peers = __ballot_sync(0xffffffffu, ok);
+#pragma unroll
+        for (int b = 0; b < kRadixBits; ++b) {
+            const uint32_t m = __ballot_sync(0xffffffffu, (d >> b) & 1u);
+            peers &= ((d >> b) & 1u) ? m : ~m;
+        }
         uint32_t prior = 0;
         if (ok) prior = warp_cnt[warp][d];
         __syncwarp();
@@ -145,23 +156,37 @@ __global__ void __launch_bounds__(kSortThreads) radix_scatter(const uint32_t* __
         __syncwarp();
     }
     __syncthreads();
+    uint32_t mine = 0;
     {   // exclusive scan over the warps, per digit
-        uint32_t run = 0;
 #pragma unroll
         for (int w = 0; w < kSortWarps; ++w) {
             const uint32_t c = warp_cnt[w][threadIdx.x];
-            warp_cnt[w][threadIdx.x] = run;
-            run += c;
+            warp_cnt[w][threadIdx.x] = mine;
+            mine += c;
         }
     }
+    tile_off[threadIdx.x] = block_exclusive_scan(mine, warp_sums, &total);                  // syncs
     __syncthreads();
 #pragma unroll
     for (int r = 0; r < kItems; ++r) {
         if (base + r * 32 + lane < n) {
             const uint32_t d = (k[r] >> shift) & (kRadix - 1);
-            const uint32_t dst = digit_base[d] + warp_cnt[warp][d] + rank[r];
-            key_out[dst] = k[r];
-            val_out[dst] = v[r];
+            const uint32_t lp = tile_off[d] + warp_cnt[warp][d] + rank[r];
+            s_key[lp] = k[r];
+            s_val[lp] = v[r];
+        }
+    }
+    __syncthreads();
+    const int n_here = (int)min((int64_t)kTile, n - tile_base);
+#pragma unroll
+    for (int r = 0; r < kItems; ++r) {
+        const int j = r * kSortThreads + threadIdx.x;
+        if (j < n_here) {
+            const uint32_t kk = s_key[j];
+            const uint32_t d = (kk >> shift) & (kRadix - 1);
+            const uint32_t dst = digit_base[d] + ((uint32_t)j - tile_off[d]);
+            key_out[dst] = kk;
+            val_out[dst] = s_val[j];
         }
     }
 }
