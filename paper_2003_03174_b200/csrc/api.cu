@@ -120,6 +120,7 @@ void trd_destroy(trd_handle* h) {
     release(h->tile_hist);
     release(h->digit_tot);
     release(h->bin_first);
+    release(h->row_ext);
     release(h->stage_tl);
     release(h->stage_in);
     release(h->stage_out);
@@ -263,7 +264,7 @@ const char* trd_last_error(const trd_handle* h) { return h ? h->err.c_str() : "N
 
 int64_t trd_device_bytes(const trd_handle* h) {
     if (!h) return 0;
-    size_t t = h->store.bytes + h->packed.bytes + h->tile_hist.bytes + h->digit_tot.bytes + h->bin_first.bytes + h->stage_tl.bytes +
+    size_t t = h->store.bytes + h->packed.bytes + h->tile_hist.bytes + h->digit_tot.bytes + h->bin_first.bytes + h->row_ext.bytes + h->stage_tl.bytes +
                h->stage_in.bytes + h->stage_out.bytes + h->trk_rec.bytes + h->trk_out.bytes + h->trk_hist.bytes +
                h->trk_tot.bytes;
     for (int s = 0; s < 2; ++s) t += h->key[s].bytes + h->val[s].bytes + h->trk_key[s].bytes + h->trk_val[s].bytes;

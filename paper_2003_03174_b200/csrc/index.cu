@@ -191,11 +191,43 @@ __global__ void __launch_bounds__(kSortThreads) radix_scatter(const uint32_t* __
     }
 }
 
-__global__ void __launch_bounds__(256) gather_store(const uint32_t* __restrict__ pos, const float4* __restrict__ packed,
-                                                    float4* __restrict__ store, int64_t n) {
+__device__ __forceinline__ uint32_t ext_encode(float f) {          // order-preserving float -> uint
+    const uint32_t b = __float_as_uint(f);
+    return (b & 0x80000000u) ? ~b : (b ^ 0x80000000u);
+}
+
+// also records the z extent of every (cell, z row): row_ext[row] = (min, max) of the encoded z.  The keys are
+// sorted, so a warp almost always lies inside one row: one warp reduction and two atomics per warp.
+__global__ void __launch_bounds__(256) gather_store(const uint32_t* __restrict__ pos, const uint32_t* __restrict__ key,
+                                                    const float4* __restrict__ packed, float4* __restrict__ store,
+                                                    uint2* __restrict__ row_ext, int64_t n, uint32_t n_bins, int nb_shift) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    store[i] = __ldg(packed + pos[i]);
+    const bool ok = i < n;
+    uint32_t row = 0xffffffffu, zlo = 0xffffffffu, zhi = 0u;
+    if (ok) {
+        const float4 tl = __ldg(packed + pos[i]);
+        store[i] = tl;
+        const uint32_t k = key[i];
+        if (k < n_bins) {
+            row = k >> nb_shift;
+            zlo = zhi = ext_encode(tl.y);
+        }
+    }
+    const uint32_t row0 = __shfl_sync(0xffffffffu, row, 0);
+    if (__all_sync(0xffffffffu, row == row0)) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            zlo = min(zlo, __shfl_xor_sync(0xffffffffu, zlo, o));
+            zhi = max(zhi, __shfl_xor_sync(0xffffffffu, zhi, o));
+        }
+        if ((threadIdx.x & 31) == 0 && row != 0xffffffffu) {
+            atomicMin(&row_ext[row].x, zlo);
+            atomicMax(&row_ext[row].y, zhi);
+        }
+    } else if (row != 0xffffffffu) {
+        atomicMin(&row_ext[row].x, zlo);
+        atomicMax(&row_ext[row].y, zhi);
+    }
 }
 
 // bin_first[b] = first sorted position whose key is >= b, for b = 0..n_bins
@@ -298,6 +330,11 @@ cudaError_t build_index(trd_handle* h, const float* d_y, const float* d_z, const
     h->index_loaded = false;
 
     TRD_TRY(reserve(h->bin_first, ((size_t)g.n_bins + 1) * sizeof(int32_t), stream));
+    const size_t n_rows = (size_t)n_cells * g.nz;
+    TRD_TRY(reserve(h->row_ext, n_rows * sizeof(uint2), stream));
+    // empty rows: min = 0xffffffff > max = 0
+    TRD_TRY(cudaMemset2DAsync(h->row_ext.p, sizeof(uint2), 0xff, sizeof(uint32_t), n_rows, stream));
+    TRD_TRY(cudaMemset2DAsync((char*)h->row_ext.p + sizeof(uint32_t), sizeof(uint2), 0x00, sizeof(uint32_t), n_rows, stream));
     if (n == 0) {
         TRD_TRY(cudaMemsetAsync(h->bin_first.p, 0, ((size_t)g.n_bins + 1) * sizeof(int32_t), stream));
         h->index_loaded = true;
@@ -320,7 +357,9 @@ cudaError_t build_index(trd_handle* h, const float* d_y, const float* d_z, const
     TRD_TRY(radix_sort_pairs((uint32_t*)h->key[0].p, (uint32_t*)h->key[1].p, (uint32_t*)h->val[0].p, (uint32_t*)h->val[1].p,
                              (uint32_t*)h->tile_hist.p, (uint32_t*)h->digit_tot.p, n, h->n_passes, stream, &side, &h->launches));
     h->sorted_side = side;
-    gather_store<<<n_blk, 256, 0, stream>>>((const uint32_t*)h->val[side].p, (const float4*)h->packed.p, (float4*)h->store.p, n);
+    gather_store<<<n_blk, 256, 0, stream>>>((const uint32_t*)h->val[side].p, (const uint32_t*)h->key[side].p,
+                                           (const float4*)h->packed.p, (float4*)h->store.p, (uint2*)h->row_ext.p, n, g.n_bins,
+                                           g.nb_shift);
     bin_first_kernel<<<n_blk, 256, 0, stream>>>((const uint32_t*)h->key[side].p, (int32_t*)h->bin_first.p, n, g.n_bins);
     h->launches += 2;
     TRD_TRY(cudaGetLastError());

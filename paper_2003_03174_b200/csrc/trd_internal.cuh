@@ -74,6 +74,7 @@ struct trd_handle {
     trd::Buffer tile_hist;  // [256][n_tiles] digit counts per tile
     trd::Buffer digit_tot;  // [256]
     trd::Buffer bin_first;  // [n_bins + 1]
+    trd::Buffer row_ext;    // uint2 per (cell, z row): encoded min and max z of the row
     int sorted_side = 0;    // which of key[]/val[] holds the sorted result
     // staging for the *_host entry points
     trd::Buffer stage_tl;   // tracklets
