@@ -154,6 +154,9 @@ int trd_copy_index(trd_handle* h, int32_t* sorted_pos, uint32_t* sorted_key, int
 const char* trd_last_error(const trd_handle* h);
 int64_t trd_device_bytes(const trd_handle* h);   /* device memory currently owned by the handle */
 int64_t trd_kernel_launches(const trd_handle* h); /* kernels launched through this handle so far */
+/* Device time of the match kernel alone in the most recent trd_match (CUDA events recorded on the call's
+ * stream around that one launch; waits for the end event).  TRD_E_STATE if no trd_match has run. */
+int trd_last_match_kernel_ms(trd_handle* h, float* ms);
 
 #ifdef __cplusplus
 }

@@ -22,7 +22,7 @@ _STATUS = {0: "TRD_OK", -1: "TRD_E_ARG", -2: "TRD_E_CUDA", -3: "TRD_E_NOMEM", -4
 
 EXPORTS = ("trd_version", "trd_create", "trd_destroy", "trd_load_tracklets", "trd_match",
            "trd_load_tracklets_host", "trd_match_host", "trd_get_index_info", "trd_copy_index",
-           "trd_last_error", "trd_device_bytes", "trd_kernel_launches")
+           "trd_last_error", "trd_device_bytes", "trd_kernel_launches", "trd_last_match_kernel_ms")
 
 _fp = C.POINTER(C.c_float)
 _ip = C.POINTER(C.c_int32)
@@ -91,6 +91,7 @@ def lib():
         l.trd_device_bytes.restype = C.c_int64
         l.trd_kernel_launches.argtypes = [C.c_void_p]
         l.trd_kernel_launches.restype = C.c_int64
+        l.trd_last_match_kernel_ms.argtypes = [C.c_void_p, C.POINTER(C.c_float)]
         _lib = l
     return _lib
 
@@ -277,6 +278,12 @@ def trd_device_bytes(h) -> int:
 
 def trd_kernel_launches(h) -> int:
     return int(lib().trd_kernel_launches(h))
+
+
+def trd_last_match_kernel_ms(h) -> float:
+    ms = C.c_float()
+    _check(h, lib().trd_last_match_kernel_ms(h, C.byref(ms)))
+    return float(ms.value)
 
 
 # ---- convenience -----------------------------------------------------------------------------

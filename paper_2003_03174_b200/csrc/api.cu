@@ -132,6 +132,8 @@ void trd_destroy(trd_handle* h) {
     }
     release(h->trk_hist);
     release(h->trk_tot);
+    for (int k = 0; k < 2; ++k)
+        if (h->ev_match[k]) cudaEventDestroy(h->ev_match[k]);
     delete h;
 }
 
@@ -272,5 +274,14 @@ int64_t trd_device_bytes(const trd_handle* h) {
 }
 
 int64_t trd_kernel_launches(const trd_handle* h) { return h ? h->launches : 0; }
+
+int trd_last_match_kernel_ms(trd_handle* h, float* ms) {
+    if (!h || !ms) return TRD_E_ARG;
+    if (!h->ev_recorded) return fail(h, TRD_E_STATE, "trd_last_match_kernel_ms: no trd_match has run");
+    cudaError_t e = cudaEventSynchronize(h->ev_match[1]);
+    if (e == cudaSuccess) e = cudaEventElapsedTime(ms, h->ev_match[0], h->ev_match[1]);
+    if (e != cudaSuccess) return fail_cuda(h, e, "trd_last_match_kernel_ms");
+    return TRD_OK;
+}
 
 }  // extern "C"

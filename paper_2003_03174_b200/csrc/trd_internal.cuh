@@ -65,6 +65,8 @@ struct trd_handle {
     int key_bits = 0, n_passes = 0;
     double ybin_width = 0.0;
     int64_t launches = 0;
+    cudaEvent_t ev_match[2] = {nullptr, nullptr};   // around the match kernel of the last trd_match
+    bool ev_recorded = false;
     std::string err;
     // device buffers owned by the handle
     trd::Buffer store;      // float4 per sorted tracklet: y, z, dy/dx, original position (bits)
