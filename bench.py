@@ -113,6 +113,15 @@ def load_units(spec, n_batches):
     return u["batches"]
 
 
+def config_dict(spec, n_tl, world):
+    n, batch = spec.n_tracks, spec.batch or spec.n_tracks
+    nb = (n + batch - 1) // batch
+    return dict(workload=spec.name, n_tracks=n, n_tracklets=n_tl, n_hyp=spec.n_hyp, n_sigma_road=spec.n_sigma_road,
+                batch=batch, step="1 trd_load_tracklets + %d trd_match" % nb,
+                l2="inputs larger than L2 (%.0f MB tracklets + %.0f MB tracks per step)" % (16e-6 * n_tl, 88e-6 * n),
+                parallelism=f"{world} x independent time frames, no collective")
+
+
 def oracle_sample(cfg, data, n_sample, n_threads=0):
     """The oracle, as it stands, on the first n_sample tracks against ALL tracklets."""
     from oracle import oracle as O
@@ -145,8 +154,7 @@ def run_reference(args, spec, cfg):
     line = dict(impl="reference", metric=METRIC, value=value, unit=UNIT, n_gpus=args.gpus, steps=args.steps,
                 warmup=args.warmup, ms_per_step=1e3 * wall / max(args.steps, 1), higher_is_better=True, scaling="weak",
                 vs_baseline=None, dtype="f64", data="synthetic",
-                config=dict(workload=spec.name, n_tracks=spec.n_tracks, n_tracklets=int(data["tl_y"].shape[0]),
-                            n_hyp=spec.n_hyp, n_sigma_road=spec.n_sigma_road),
+                config=config_dict(spec, int(data["tl_y"].shape[0]), max(args.gpus, 1)),
                 cpu_baseline=dict(value=value, unit=UNIT, cores=cores, kind="oracle", sample=sample),
                 e2e=dict(value=value, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0), gpu_launches=0)
     print(json.dumps(line), flush=True)
@@ -291,10 +299,7 @@ def run_ours(args, spec, cfg):
     line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=max(args.warmup, 3),
                 ms_per_step=ms_per_step, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32",
                 data="synthetic",
-                config=dict(workload=spec.name, n_tracks=n, n_tracklets=n_tl, n_hyp=spec.n_hyp, n_sigma_road=spec.n_sigma_road,
-                            batch=batch, step="1 trd_load_tracklets + %d trd_match" % nb,
-                            l2="inputs larger than L2 (%.0f MB tracklets + %.0f MB tracks per step)" % (16e-6 * n_tl, 88e-6 * n),
-                            parallelism=f"{world} x independent time frames, no collective"),
+                config=config_dict(spec, n_tl, world),
                 cand_evals_per_s=world * n_evals / (ms_per_step * 1e-3), n_cand_evals=n_evals,
                 frac_tracks_ge2_tracklets=n_ge2 / n, index=dict(n_ybins=info["n_ybins"], n_zrows=info["n_zrows"],
                                                                 ybin_width_cm=info["ybin_width"], radix_passes=info["n_passes"]),
