@@ -237,7 +237,8 @@ def run_ours(args, spec, cfg):
     def step_host():
         B.trd_load_tracklets_host(h, *h_tl, stream=stream)
         for t, o in zip(h_tracks, h_outs):
-            B.trd_match_host(h, t, o, stream=stream)
+            B.trd_match_host_async(h, t, o, stream=stream)
+        B.trd_wait_host(h, stream=stream)            # results of all batches are in host memory here
 
     for _ in range(2):
         step_host()

@@ -138,11 +138,21 @@ int trd_load_tracklets(trd_handle* h, const float* d_y, const float* d_z, const 
 int trd_match(trd_handle* h, const trd_tracks_in* in, const trd_tracks_out* out, int64_t n_tracks,
               void* stream);
 
-/* Same two calls with HOST arrays: the library copies the inputs to its own device buffers
- * on `stream`, runs the same kernels, copies the outputs back and synchronises `stream`
- * before returning (trd_load_tracklets_host returns without waiting for the kernels). */
+/* The same two calls with HOST arrays (pinned memory makes the copies asynchronous; pageable memory works
+ * too).  The library stages through its own device buffers and pipelines on two internal copy streams:
+ * host->device copies, the kernels (on `stream`) and device->host copies of consecutive calls overlap.
+ *   trd_load_tracklets_host   returns once the copies and kernels are queued; the arrays must stay valid
+ *                             until trd_wait_host has returned;
+ *   trd_match_host_async      queues copy-in, trd_match and copy-out of one batch and returns; the results
+ *                             are in `out_host` only after trd_wait_host.  At most two batches are in flight:
+ *                             a third call first waits for the oldest;
+ *   trd_wait_host             blocks until everything queued by *_host calls has completed;
+ *   trd_match_host            = trd_match_host_async + trd_wait_host. */
 int trd_load_tracklets_host(trd_handle* h, const float* y, const float* z, const float* dydx,
                             const int32_t* chamber, int64_t n, void* stream);
+int trd_match_host_async(trd_handle* h, const trd_tracks_in* in_host, const trd_tracks_out* out_host,
+                         int64_t n_tracks, void* stream);
+int trd_wait_host(trd_handle* h, void* stream);
 int trd_match_host(trd_handle* h, const trd_tracks_in* in_host, const trd_tracks_out* out_host,
                    int64_t n_tracks, void* stream);
 

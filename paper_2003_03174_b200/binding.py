@@ -21,7 +21,7 @@ TRD_OK, TRD_E_ARG, TRD_E_CUDA, TRD_E_NOMEM, TRD_E_STATE = 0, -1, -2, -3, -4
 _STATUS = {0: "TRD_OK", -1: "TRD_E_ARG", -2: "TRD_E_CUDA", -3: "TRD_E_NOMEM", -4: "TRD_E_STATE"}
 
 EXPORTS = ("trd_version", "trd_create", "trd_destroy", "trd_load_tracklets", "trd_match",
-           "trd_load_tracklets_host", "trd_match_host", "trd_get_index_info", "trd_copy_index",
+           "trd_load_tracklets_host", "trd_match_host", "trd_match_host_async", "trd_wait_host", "trd_get_index_info", "trd_copy_index",
            "trd_last_error", "trd_device_bytes", "trd_kernel_launches", "trd_last_match_kernel_ms")
 
 _fp = C.POINTER(C.c_float)
@@ -83,6 +83,8 @@ def lib():
         l.trd_load_tracklets_host.argtypes = l.trd_load_tracklets.argtypes
         l.trd_match.argtypes = [C.c_void_p, C.POINTER(TrdTracksIn), C.POINTER(TrdTracksOut), C.c_int64, C.c_void_p]
         l.trd_match_host.argtypes = l.trd_match.argtypes
+        l.trd_match_host_async.argtypes = l.trd_match.argtypes
+        l.trd_wait_host.argtypes = [C.c_void_p, C.c_void_p]
         l.trd_get_index_info.argtypes = [C.c_void_p, C.POINTER(TrdIndexInfo)]
         l.trd_copy_index.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         l.trd_last_error.argtypes = [C.c_void_p]
@@ -231,7 +233,16 @@ def alloc_tracks_out_host(n: int, pinned: bool = False) -> Dict[str, np.ndarray]
     return out
 
 
-def trd_match_host(h, tracks: dict, out: Optional[dict] = None, stream=None) -> dict:
+def trd_wait_host(h, stream=None) -> None:
+    _check(h, lib().trd_wait_host(h, _stream(stream)))
+
+
+def trd_match_host_async(h, tracks: dict, out: Optional[dict] = None, stream=None) -> dict:
+    """trd_match_host without the final wait: `out` is valid only after trd_wait_host (pinned arrays overlap)."""
+    return trd_match_host(h, tracks, out, stream, _async=True)
+
+
+def trd_match_host(h, tracks: dict, out: Optional[dict] = None, stream=None, _async: bool = False) -> dict:
     """Same as trd_match with numpy arrays; returns when the results are in `out`."""
     n = tracks["x"].size
     if out is None:
@@ -253,7 +264,8 @@ def trd_match_host(h, tracks: dict, out: Optional[dict] = None, stream=None) -> 
         tout.chi2 = _host_ptr(out["chi2"], np.float32, n)
         tout.n_matched = _host_ptr(out["n_matched"], np.int32, n)
         tout.n_cand_evals = _host_ptr(out["n_evals"], np.int32, n) if "n_evals" in out else None
-    _check(h, lib().trd_match_host(h, C.byref(tin), C.byref(tout), n, _stream(stream)))
+    fn = lib().trd_match_host_async if _async else lib().trd_match_host
+    _check(h, fn(h, C.byref(tin), C.byref(tout), n, _stream(stream)))
     return out
 
 

@@ -8,7 +8,7 @@
 
 #include "trd_internal.cuh"
 
-namespace {
+namespace trd {
 
 int fail(trd_handle* h, int code, const std::string& what) {
     if (h) h->err = what;
@@ -20,6 +20,13 @@ int fail_cuda(trd_handle* h, cudaError_t e, const char* where) {
     const int code = (e == cudaErrorMemoryAllocation) ? TRD_E_NOMEM : TRD_E_CUDA;
     return fail(h, code, std::string(where) + ": " + cudaGetErrorString(e));
 }
+
+}  // namespace trd
+
+namespace {
+
+using trd::fail;
+using trd::fail_cuda;
 
 bool derive_params(const trd_config& c, trd::MatchParams& mp) {
     memset(&mp, 0, sizeof mp);
@@ -79,8 +86,6 @@ void release(trd::Buffer& b) {
     b.bytes = 0;
 }
 
-constexpr int kInArrays = 5 + 15 + 1 + 1;                    // par, cov, x, sector
-constexpr int kOutArrays = TRD_MAX_LAYERS + 5 + 15 + 5;      // idx, par, cov, x, sector, chi2, n_matched, n_cand_evals
 
 }  // namespace
 
@@ -121,9 +126,7 @@ void trd_destroy(trd_handle* h) {
     release(h->digit_tot);
     release(h->bin_first);
     release(h->row_ext);
-    release(h->stage_tl);
-    release(h->stage_in);
-    release(h->stage_out);
+    trd::host_pipeline_destroy(h);
     release(h->trk_rec);
     release(h->trk_out);
     for (int s = 0; s < 2; ++s) {
@@ -165,74 +168,6 @@ int trd_match(trd_handle* h, const trd_tracks_in* in, const trd_tracks_out* out,
     return TRD_OK;
 }
 
-int trd_load_tracklets_host(trd_handle* h, const float* y, const float* z, const float* dydx,
-                            const int32_t* chamber, int64_t n, void* stream) {
-    if (!h) return TRD_E_ARG;
-    if (n < 0 || n >= (1 << 29) - 1) return fail(h, TRD_E_ARG, "trd_load_tracklets_host: n out of range (must be < 2^29 - 1)");
-    if (n > 0 && (!y || !z || !dydx || !chamber)) return fail(h, TRD_E_ARG, "trd_load_tracklets_host: NULL array");
-    cudaStream_t st = (cudaStream_t)stream;
-    const size_t bytes = (size_t)n * 4;
-    cudaError_t e = trd::reserve(h->stage_tl, 4 * bytes + 16, st);
-    if (e != cudaSuccess) return fail_cuda(h, e, "trd_load_tracklets_host");
-    char* base = (char*)h->stage_tl.p;
-    const void* src[4] = {y, z, dydx, chamber};
-    for (int k = 0; k < 4 && n > 0; ++k) {
-        e = cudaMemcpyAsync(base + k * bytes, src[k], bytes, cudaMemcpyHostToDevice, st);
-        if (e != cudaSuccess) return fail_cuda(h, e, "trd_load_tracklets_host: copy");
-    }
-    return trd_load_tracklets(h, (const float*)base, (const float*)(base + bytes), (const float*)(base + 2 * bytes),
-                              (const int32_t*)(base + 3 * bytes), n, stream);
-}
-
-int trd_match_host(trd_handle* h, const trd_tracks_in* in, const trd_tracks_out* out, int64_t n, void* stream) {
-    if (!h) return TRD_E_ARG;
-    if (!in || !out || n < 0) return fail(h, TRD_E_ARG, "trd_match_host: NULL struct or negative n_tracks");
-    if (!h->index_loaded) return fail(h, TRD_E_STATE, "trd_match_host: no tracklets loaded");
-    if (n == 0) return TRD_OK;
-    cudaStream_t st = (cudaStream_t)stream;
-    const size_t bytes = (size_t)n * 4;
-    cudaError_t e = trd::reserve(h->stage_in, kInArrays * bytes, st);
-    if (e == cudaSuccess) e = trd::reserve(h->stage_out, kOutArrays * bytes, st);
-    if (e != cudaSuccess) return fail_cuda(h, e, "trd_match_host");
-    char* bi = (char*)h->stage_in.p;
-    char* bo = (char*)h->stage_out.p;
-    trd_tracks_in din;
-    trd_tracks_out dout;
-    const void* src[kInArrays];
-    void* dst[kOutArrays];
-    int a = 0;
-    for (int k = 0; k < 5; ++k) { src[a] = in->par[k]; din.par[k] = (const float*)(bi + a * bytes); ++a; }
-    for (int k = 0; k < 15; ++k) { src[a] = in->cov[k]; din.cov[k] = (const float*)(bi + a * bytes); ++a; }
-    src[a] = in->x; din.x = (const float*)(bi + a * bytes); ++a;
-    src[a] = in->sector; din.sector = (const int32_t*)(bi + a * bytes); ++a;
-    int b = 0;
-    for (int l = 0; l < TRD_MAX_LAYERS; ++l) { dst[b] = out->tracklet_idx[l]; dout.tracklet_idx[l] = (int32_t*)(bo + b * bytes); ++b; }
-    for (int k = 0; k < 5; ++k) { dst[b] = out->par[k]; dout.par[k] = (float*)(bo + b * bytes); ++b; }
-    for (int k = 0; k < 15; ++k) { dst[b] = out->cov[k]; dout.cov[k] = (float*)(bo + b * bytes); ++b; }
-    dst[b] = out->x; dout.x = (float*)(bo + b * bytes); ++b;
-    dst[b] = out->sector; dout.sector = (int32_t*)(bo + b * bytes); ++b;
-    dst[b] = out->chi2; dout.chi2 = (float*)(bo + b * bytes); ++b;
-    dst[b] = out->n_matched; dout.n_matched = (int32_t*)(bo + b * bytes); ++b;
-    dst[b] = out->n_cand_evals; dout.n_cand_evals = out->n_cand_evals ? (int32_t*)(bo + b * bytes) : nullptr; ++b;
-    for (int k = 0; k < kInArrays; ++k) {
-        if (!src[k]) return fail(h, TRD_E_ARG, "trd_match_host: NULL input array");
-        e = cudaMemcpyAsync(bi + k * bytes, src[k], bytes, cudaMemcpyHostToDevice, st);
-        if (e != cudaSuccess) return fail_cuda(h, e, "trd_match_host: copy in");
-    }
-    for (int k = 0; k < kOutArrays - 1; ++k)
-        if (!dst[k]) return fail(h, TRD_E_ARG, "trd_match_host: NULL output array");
-    const int rc = trd_match(h, &din, &dout, n, stream);
-    if (rc != TRD_OK) return rc;
-    for (int k = 0; k < kOutArrays; ++k) {
-        if (!dst[k]) continue;
-        e = cudaMemcpyAsync(dst[k], bo + k * bytes, bytes, cudaMemcpyDeviceToHost, st);
-        if (e != cudaSuccess) return fail_cuda(h, e, "trd_match_host: copy out");
-    }
-    e = cudaStreamSynchronize(st);
-    if (e != cudaSuccess) return fail_cuda(h, e, "trd_match_host: synchronize");
-    return TRD_OK;
-}
-
 int trd_get_index_info(const trd_handle* h, trd_index_info* info) {
     if (!h || !info) return TRD_E_ARG;
     if (!h->index_loaded) return TRD_E_STATE;
@@ -266,8 +201,7 @@ const char* trd_last_error(const trd_handle* h) { return h ? h->err.c_str() : "N
 
 int64_t trd_device_bytes(const trd_handle* h) {
     if (!h) return 0;
-    size_t t = h->store.bytes + h->packed.bytes + h->tile_hist.bytes + h->digit_tot.bytes + h->bin_first.bytes + h->row_ext.bytes + h->stage_tl.bytes +
-               h->stage_in.bytes + h->stage_out.bytes + h->trk_rec.bytes + h->trk_out.bytes + h->trk_hist.bytes +
+    size_t t = h->store.bytes + h->packed.bytes + h->tile_hist.bytes + h->digit_tot.bytes + h->bin_first.bytes + h->row_ext.bytes + h->stage_tl.bytes + h->trk_rec.bytes + h->trk_out.bytes + h->trk_hist.bytes +
                h->trk_tot.bytes;
     for (int s = 0; s < 2; ++s) t += h->key[s].bytes + h->val[s].bytes + h->trk_key[s].bytes + h->trk_val[s].bytes;
     return (int64_t)t;

@@ -80,8 +80,15 @@ struct trd_handle {
     int sorted_side = 0;    // which of key[]/val[] holds the sorted result
     // staging for the *_host entry points
     trd::Buffer stage_tl;   // tracklets
-    trd::Buffer stage_in;   // tracks in
-    trd::Buffer stage_out;  // tracks out
+    // pipelined host entry points (host_api.cu): own copy streams, a ring of staging slots
+    static constexpr int kRing = 2;
+    cudaStream_t s_in = nullptr, s_out = nullptr;        // host->device and device->host copy streams
+    trd::Buffer stage_in[kRing], stage_out[kRing];       // tracks in / out per ring slot
+    cudaEvent_t ev_in[kRing] = {}, ev_done[kRing] = {}, ev_out[kRing] = {};   // copied in / matched / copied out
+    bool slot_busy[kRing] = {};
+    cudaEvent_t ev_tl_in = nullptr, ev_tl_used = nullptr;  // tracklets copied in / consumed by the index build
+    bool tl_pending = false;
+    int ring_next = 0;
     // track binning (trd_match on large batches): packed records and the permutation
     trd::Buffer trk_rec;    // kRecIn floats per track, caller's order
     trd::Buffer trk_out;    // kRecOut floats per track, caller's order
@@ -111,6 +118,10 @@ cudaError_t radix_sort_pairs(uint32_t* key0, uint32_t* key1, uint32_t* val0, uin
 cudaError_t pack_tracks(trd_handle* h, const trd_tracks_in& in, int64_t n, float* rec, uint32_t* key, int* key_bits,
                         cudaStream_t stream);
 cudaError_t unpack_tracks(trd_handle* h, const float* rec_out, const trd_tracks_out& out, int64_t n, cudaStream_t stream);
+
+int fail(trd_handle* h, int code, const std::string& what);
+int fail_cuda(trd_handle* h, cudaError_t e, const char* where);
+void host_pipeline_destroy(trd_handle* h);
 
 // grows b to at least `bytes` (contents lost); synchronises `stream` before freeing
 cudaError_t reserve(Buffer& b, size_t bytes, cudaStream_t stream);

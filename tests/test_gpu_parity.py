@@ -217,3 +217,31 @@ def test_track_binning_does_not_change_results(B, name):
         np.testing.assert_array_equal(on_ragged[k], off[k])
     want = O.match(cfg, d)
     assert_parity(P.compare(on, want), want)
+
+
+def test_pipelined_host_entry_points(B):
+    """trd_match_host_async + trd_wait_host: five batches through the two-slot ring (the third call has to
+    retire the first), pinned and pageable buffers, two consecutive loads on one handle; bit-equal to the
+    device entry points."""
+    spec = W.CONFIGS["pileup"]; d = W.generate(spec); cfg = dict(W.matcher_config(spec), track_binning=1)
+    want = run_gpu(B, cfg, d)
+    n = spec.n_tracks
+    bounds = [(lo, min(n, lo + 5003)) for lo in range(0, n, 5003)]
+    h = B.trd_create(cfg)
+    try:
+        for pinned in (True, False):
+            B.trd_load_tracklets_host(h, d["tl_y"][:1000].copy(), d["tl_z"][:1000].copy(), d["tl_dydx"][:1000].copy(),
+                                      d["tl_chamber"][:1000].copy())          # superseded by the next load
+            B.trd_load_tracklets_host(h, d["tl_y"], d["tl_z"], d["tl_dydx"], d["tl_chamber"])
+            ins = [dict(par=np.ascontiguousarray(d["par"][:, lo:hi]), cov=np.ascontiguousarray(d["cov"][:, lo:hi]),
+                        x=np.ascontiguousarray(d["x"][lo:hi]), sector=np.ascontiguousarray(d["sector"][lo:hi]))
+                   for lo, hi in bounds]
+            outs = [B.alloc_tracks_out_host(hi - lo, pinned=pinned) for lo, hi in bounds]
+            for t, o in zip(ins, outs):
+                B.trd_match_host_async(h, t, o)
+            B.trd_wait_host(h)
+            for k in ("idx", "par", "cov", "x", "sector", "chi2", "n_matched", "n_evals"):
+                got = np.concatenate([o[k] for o in outs], axis=-1)
+                np.testing.assert_array_equal(got, want[k])
+    finally:
+        B.trd_destroy(h)
