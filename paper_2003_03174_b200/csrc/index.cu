@@ -4,7 +4,7 @@
 //   a2  radix_*          stable LSD radix sort of (key, position), 8 bits per pass:
 //                        per-tile digit histogram -> per-digit scan over tiles -> stable scatter
 //       gather_store     sorted store: one float4 (y, z, dy/dx, position) per tracklet
-//   a3  bin_first        first sorted position of every bin (plus sentinel)
+//   a3  (in gather_store) first sorted position of every bin (plus sentinel), z extent of every row
 //
 // north_star: "device-side sort and index by chamber and local-y bin ... a radix sort plus
 // per-chamber y-bin offsets"; the 18 x 5 x 6 segmentation is PAPER.md:50.  The key also
@@ -200,7 +200,8 @@ __device__ __forceinline__ uint32_t ext_encode(float f) {          // order-pres
 // sorted, so a warp almost always lies inside one row: one warp reduction and two atomics per warp.
 __global__ void __launch_bounds__(256) gather_store(const uint32_t* __restrict__ pos, const uint32_t* __restrict__ key,
                                                     const float4* __restrict__ packed, float4* __restrict__ store,
-                                                    uint2* __restrict__ row_ext, int64_t n, uint32_t n_bins, int nb_shift) {
+                                                    uint2* __restrict__ row_ext, int32_t* __restrict__ bin_first, int64_t n,
+                                                    uint32_t n_bins, int nb_shift) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const bool ok = i < n;
     uint32_t row = 0xffffffffu, zlo = 0xffffffffu, zhi = 0u;
@@ -208,6 +209,13 @@ __global__ void __launch_bounds__(256) gather_store(const uint32_t* __restrict__
         const float4 tl = __ldg(packed + pos[i]);
         store[i] = tl;
         const uint32_t k = key[i];
+        {   // a3: bin_first[b] = first sorted position whose key is >= b, for b = 0..n_bins (boundary detection)
+            const uint32_t kc = min(k, n_bins);
+            const int64_t lo = (i == 0) ? 0 : (int64_t)min(key[i - 1], n_bins) + 1;
+            for (int64_t b = lo; b <= (int64_t)kc; ++b) bin_first[b] = (int32_t)i;
+            if (i == n - 1)
+                for (int64_t b = (int64_t)kc + 1; b <= (int64_t)n_bins; ++b) bin_first[b] = (int32_t)n;
+        }
         if (k < n_bins) {
             row = k >> nb_shift;
             zlo = zhi = ext_encode(tl.y);
@@ -228,18 +236,6 @@ __global__ void __launch_bounds__(256) gather_store(const uint32_t* __restrict__
         atomicMin(&row_ext[row].x, zlo);
         atomicMax(&row_ext[row].y, zhi);
     }
-}
-
-// bin_first[b] = first sorted position whose key is >= b, for b = 0..n_bins
-__global__ void __launch_bounds__(256) bin_first_kernel(const uint32_t* __restrict__ key, int32_t* __restrict__ bin_first,
-                                                        int64_t n, uint32_t n_bins) {
-    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    const uint32_t k = min(key[i], n_bins);
-    const int64_t lo = (i == 0) ? 0 : (int64_t)min(key[i - 1], n_bins) + 1;
-    for (int64_t b = lo; b <= (int64_t)k; ++b) bin_first[b] = (int32_t)i;
-    if (i == n - 1)
-        for (int64_t b = (int64_t)k + 1; b <= (int64_t)n_bins; ++b) bin_first[b] = (int32_t)n;
 }
 
 inline int ceil_log2(uint64_t v) {
@@ -358,10 +354,9 @@ cudaError_t build_index(trd_handle* h, const float* d_y, const float* d_z, const
                              (uint32_t*)h->tile_hist.p, (uint32_t*)h->digit_tot.p, n, h->n_passes, stream, &side, &h->launches));
     h->sorted_side = side;
     gather_store<<<n_blk, 256, 0, stream>>>((const uint32_t*)h->val[side].p, (const uint32_t*)h->key[side].p,
-                                           (const float4*)h->packed.p, (float4*)h->store.p, (uint2*)h->row_ext.p, n, g.n_bins,
-                                           g.nb_shift);
-    bin_first_kernel<<<n_blk, 256, 0, stream>>>((const uint32_t*)h->key[side].p, (int32_t*)h->bin_first.p, n, g.n_bins);
-    h->launches += 2;
+                                           (const float4*)h->packed.p, (float4*)h->store.p, (uint2*)h->row_ext.p,
+                                           (int32_t*)h->bin_first.p, n, g.n_bins, g.nb_shift);
+    h->launches += 1;
     TRD_TRY(cudaGetLastError());
     h->index_loaded = true;
     return cudaSuccess;
