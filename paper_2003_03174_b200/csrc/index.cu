@@ -106,7 +106,7 @@ __global__ void __launch_bounds__(kSortThreads) radix_rowscan(uint32_t* __restri
 // stable scatter of one tile.  Order inside a tile is (warp, round, lane): warp w owns the
 // contiguous keys [w * kItems * 32, (w + 1) * kItems * 32) of the tile.  The tile is first reordered by
 // digit in shared memory so that the global writes go out as contiguous runs per digit.
-__global__ void __launch_bounds__(kSortThreads) radix_scatter(const uint32_t* __restrict__ key_in,
+__global__ void __launch_bounds__(kSortThreads, 3) radix_scatter(const uint32_t* __restrict__ key_in,
                                                               const uint32_t* __restrict__ val_in,
                                                               uint32_t* __restrict__ key_out, uint32_t* __restrict__ val_out,
                                                               const uint32_t* __restrict__ hist,
