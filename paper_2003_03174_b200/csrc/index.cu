@@ -197,44 +197,60 @@ __device__ __forceinline__ uint32_t ext_encode(float f) {          // order-pres
 }
 
 // also records the z extent of every (cell, z row): row_ext[row] = (min, max) of the encoded z.  The keys are
-// sorted, so a warp almost always lies inside one row: one warp reduction and two atomics per warp.
+// sorted, so a warp almost always lies inside one row: one warp reduction and two atomics per warp.  Each
+// thread handles kGather tracklets (independent random 16-byte reads in flight), strided by the block size.
+constexpr int kGather = 4;
+
 __global__ void __launch_bounds__(256) gather_store(const uint32_t* __restrict__ pos, const uint32_t* __restrict__ key,
                                                     const float4* __restrict__ packed, float4* __restrict__ store,
                                                     uint2* __restrict__ row_ext, int32_t* __restrict__ bin_first, int64_t n,
                                                     uint32_t n_bins, int nb_shift) {
-    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    const bool ok = i < n;
-    uint32_t row = 0xffffffffu, zlo = 0xffffffffu, zhi = 0u;
-    if (ok) {
-        const float4 tl = __ldg(packed + pos[i]);
-        store[i] = tl;
-        const uint32_t k = key[i];
-        {   // a3: bin_first[b] = first sorted position whose key is >= b, for b = 0..n_bins (boundary detection)
-            const uint32_t kc = min(k, n_bins);
-            const int64_t lo = (i == 0) ? 0 : (int64_t)min(key[i - 1], n_bins) + 1;
-            for (int64_t b = lo; b <= (int64_t)kc; ++b) bin_first[b] = (int32_t)i;
-            if (i == n - 1)
-                for (int64_t b = (int64_t)kc + 1; b <= (int64_t)n_bins; ++b) bin_first[b] = (int32_t)n;
-        }
-        if (k < n_bins) {
-            row = k >> nb_shift;
-            zlo = zhi = ext_encode(tl.y);
+    const int64_t base = (int64_t)blockIdx.x * (256 * kGather) + threadIdx.x;
+    float4 tl[kGather];
+    uint32_t k[kGather], kprev[kGather];
+#pragma unroll
+    for (int u = 0; u < kGather; ++u) {
+        const int64_t i = base + u * 256;
+        if (i < n) {
+            tl[u] = __ldg(packed + pos[i]);
+            k[u] = key[i];
+            kprev[u] = (i == 0) ? 0u : key[i - 1];
         }
     }
-    const uint32_t row0 = __shfl_sync(0xffffffffu, row, 0);
-    if (__all_sync(0xffffffffu, row == row0)) {
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            zlo = min(zlo, __shfl_xor_sync(0xffffffffu, zlo, o));
-            zhi = max(zhi, __shfl_xor_sync(0xffffffffu, zhi, o));
+    for (int u = 0; u < kGather; ++u) {
+        const int64_t i = base + u * 256;
+        const bool ok = i < n;
+        uint32_t row = 0xffffffffu, zlo = 0xffffffffu, zhi = 0u;
+        if (ok) {
+            store[i] = tl[u];
+            {   // a3: bin_first[b] = first sorted position whose key is >= b, for b = 0..n_bins (boundary detection)
+                const uint32_t kc = min(k[u], n_bins);
+                const int64_t lo = (i == 0) ? 0 : (int64_t)min(kprev[u], n_bins) + 1;
+                for (int64_t b = lo; b <= (int64_t)kc; ++b) bin_first[b] = (int32_t)i;
+                if (i == n - 1)
+                    for (int64_t b = (int64_t)kc + 1; b <= (int64_t)n_bins; ++b) bin_first[b] = (int32_t)n;
+            }
+            if (k[u] < n_bins) {
+                row = k[u] >> nb_shift;
+                zlo = zhi = ext_encode(tl[u].y);
+            }
         }
-        if ((threadIdx.x & 31) == 0 && row != 0xffffffffu) {
+        const uint32_t row0 = __shfl_sync(0xffffffffu, row, 0);
+        if (__all_sync(0xffffffffu, row == row0)) {
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                zlo = min(zlo, __shfl_xor_sync(0xffffffffu, zlo, o));
+                zhi = max(zhi, __shfl_xor_sync(0xffffffffu, zhi, o));
+            }
+            if ((threadIdx.x & 31) == 0 && row != 0xffffffffu) {
+                atomicMin(&row_ext[row].x, zlo);
+                atomicMax(&row_ext[row].y, zhi);
+            }
+        } else if (row != 0xffffffffu) {
             atomicMin(&row_ext[row].x, zlo);
             atomicMax(&row_ext[row].y, zhi);
         }
-    } else if (row != 0xffffffffu) {
-        atomicMin(&row_ext[row].x, zlo);
-        atomicMax(&row_ext[row].y, zhi);
     }
 }
 
@@ -353,7 +369,7 @@ cudaError_t build_index(trd_handle* h, const float* d_y, const float* d_z, const
     TRD_TRY(radix_sort_pairs((uint32_t*)h->key[0].p, (uint32_t*)h->key[1].p, (uint32_t*)h->val[0].p, (uint32_t*)h->val[1].p,
                              (uint32_t*)h->tile_hist.p, (uint32_t*)h->digit_tot.p, n, h->n_passes, stream, &side, &h->launches));
     h->sorted_side = side;
-    gather_store<<<n_blk, 256, 0, stream>>>((const uint32_t*)h->val[side].p, (const uint32_t*)h->key[side].p,
+    gather_store<<<(unsigned)((n + 256 * kGather - 1) / (256 * kGather)), 256, 0, stream>>>((const uint32_t*)h->val[side].p, (const uint32_t*)h->key[side].p,
                                            (const float4*)h->packed.p, (float4*)h->store.p, (uint2*)h->row_ext.p,
                                            (int32_t*)h->bin_first.p, n, g.n_bins, g.nb_shift);
     h->launches += 1;
