@@ -29,6 +29,8 @@ class OrcConfig(C.Structure):
         ("sigma_y", C.c_double), ("sigma_z", C.c_double), ("sigma_dydx", C.c_double),
         ("n_sigma_road", C.c_double), ("n_sigma_angle", C.c_double),
         ("chi2_cut", C.c_double), ("chi2_penalty", C.c_double), ("max_snp", C.c_double),
+        ("sy_c0", C.c_double), ("sy_c2", C.c_double), ("sd_c0", C.c_double), ("sd_c2", C.c_double),
+        ("sin_lorentz", C.c_double), ("tan_tilt", C.c_double), ("res_model", C.c_int32), ("pad_", C.c_int32),
     ]
 
 
@@ -61,6 +63,10 @@ def make_config(cfg: dict) -> OrcConfig:
     for k in ("z_max", "pad_length", "bz_tesla", "sigma_y", "sigma_z", "sigma_dydx", "n_sigma_road",
               "n_sigma_angle", "chi2_cut", "chi2_penalty", "max_snp"):
         setattr(c, k, float(cfg[k]))
+    # measurement model of PAPER.md:62, 66 (absent keys = the constant model of the configs)
+    for k in ("sy_c0", "sy_c2", "sd_c0", "sd_c2", "sin_lorentz", "tan_tilt"):
+        setattr(c, k, float(cfg.get(k, 0.0)))
+    c.res_model = int(cfg.get("res_model", 0))
     return c
 
 
@@ -115,15 +121,15 @@ def propagate_to_layer(cfg: dict, p, c15, x, sector, x_layer):
     return bool(ok), p, c15, xx.value, sec.value
 
 
-def update(cfg: dict, p, c15, ym, zm):
+def update(cfg: dict, p, c15, ym, zm, layer: int = 0):
     p = np.array(p, float); c15 = np.array(c15, float)
-    chi2 = lib().orc_update(C.byref(make_config(cfg)), _dp(p), _dp(c15), C.c_double(ym), C.c_double(zm))
+    chi2 = lib().orc_update(C.byref(make_config(cfg)), _dp(p), _dp(c15), C.c_double(ym), C.c_double(zm), int(layer))
     return p, c15, float(chi2)
 
 
-def road(cfg: dict, p, c15):
+def road(cfg: dict, p, c15, layer: int = 0):
     p = np.array(p, float); c15 = np.array(c15, float); out = np.zeros(6)
-    lib().orc_road(C.byref(make_config(cfg)), _dp(p), _dp(c15), _dp(out))
+    lib().orc_road(C.byref(make_config(cfg)), _dp(p), _dp(c15), _dp(out), int(layer))
     return dict(road_y=out[0], road_z=out[1], tanphi=out[2], Sinv=np.array([[out[3], out[4]], [out[4], out[5]]]))
 
 

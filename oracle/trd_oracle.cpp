@@ -50,6 +50,9 @@ struct Config {
     double sigma_y, sigma_z, sigma_dydx;
     double n_sigma_road, n_sigma_angle;
     double chi2_cut, chi2_penalty, max_snp;
+    // measurement model of PAPER.md:62 (Fig. 3) and PAPER.md:66, readings [R24-R26]; res_model = 0: constants
+    double sy_c0, sy_c2, sd_c0, sd_c2, sin_lorentz, tan_tilt;
+    int32_t res_model, pad_;
 };
 
 struct Hyp {
@@ -220,22 +223,46 @@ bool propagate_to_layer(const Config& cfg, Hyp& h, double X, double* margin, Cou
     return true;
 }
 
-// ---- measurement model: m = (y, z), H = first two rows of I, R = diag(sy^2, sz^2) [R3,R10]
+// ---- measurement model: m = (y, z), H = first two rows of I [R3]
+// res_model = 0: R = diag(sy^2, sz^2), constant sigma_dydx, no tilt [R10, R19].
+// res_model = 1 (PAPER.md:62 + Fig. 3 L58) [R24-R26]: sigma_y and sigma_dydx are second-order
+// polynomials of the track's sin(phi) with their optimum at the Lorentz angle, c0 + c2 (s - sL)^2; the pads of
+// layer L are tilted by tau_L = +-tilt (alternating), so the precise coordinate (sigma_y) is across the pad and
+// the coarse one (sigma_z) along it: R = Rot(tau) diag(sy^2, sz^2) Rot(tau)^T, i.e. correlated y-z errors.  The
+// y road is applied to the residual corrected with the extrapolated z, r'_y = r_y - tan(tau) r_z, whose
+// variance is (A S A^T)_yy with A = [[1, -tan(tau)], [0, 1]]; chi2 = r^T S^-1 r is invariant under A.
 struct Road {
     double Sinv[2][2];
     double road_y, road_z, tanphi;
+    double tan_tilt, veto;
 };
 
-Road make_road(const Config& cfg, const Hyp& h) {
+Road make_road(const Config& cfg, const Hyp& h, int layer) {
     Road rd;
-    const double S00 = h.C[0][0] + cfg.sigma_y * cfg.sigma_y;
-    const double S01 = h.C[1][0];
-    const double S11 = h.C[1][1] + cfg.sigma_z * cfg.sigma_z;
+    double Ryy = cfg.sigma_y * cfg.sigma_y, Ryz = 0.0, Rzz = cfg.sigma_z * cfg.sigma_z;
+    rd.tan_tilt = 0.0;
+    rd.veto = cfg.n_sigma_angle * cfg.sigma_dydx;
+    if (cfg.res_model != 0) {
+        const double ds = h.p[2] - cfg.sin_lorentz;
+        const double sy = cfg.sy_c0 + cfg.sy_c2 * ds * ds;
+        const double sd = cfg.sd_c0 + cfg.sd_c2 * ds * ds;
+        const double t = (layer % 2 == 0) ? cfg.tan_tilt : -cfg.tan_tilt;
+        const double c2 = 1.0 / (1.0 + t * t), sz2 = cfg.sigma_z * cfg.sigma_z;
+        Ryy = c2 * (sy * sy + t * t * sz2);
+        Ryz = c2 * t * (sz2 - sy * sy);
+        Rzz = c2 * (t * t * sy * sy + sz2);
+        rd.tan_tilt = t;
+        rd.veto = cfg.n_sigma_angle * sd;
+    }
+    const double S00 = h.C[0][0] + Ryy;
+    const double S01 = h.C[1][0] + Ryz;
+    const double S11 = h.C[1][1] + Rzz;
     const double det = S00 * S11 - S01 * S01;
     rd.Sinv[0][0] = S11 / det;
     rd.Sinv[0][1] = rd.Sinv[1][0] = -S01 / det;
     rd.Sinv[1][1] = S00 / det;
-    rd.road_y = cfg.n_sigma_road * std::sqrt(S00);                                   // [R2]
+    const double t = rd.tan_tilt;
+    rd.road_y = cfg.n_sigma_road * std::sqrt(S00 - 2.0 * t * S01 + t * t * S11);     // [R2], of the corrected residual
     rd.road_z = cfg.n_sigma_road * std::sqrt(h.C[1][1]) + 0.5 * cfg.pad_length;      // [R2]
     rd.tanphi = h.p[2] / std::sqrt(1.0 - h.p[2] * h.p[2]);
     return rd;
@@ -246,8 +273,8 @@ inline double chi2_of(const Road& rd, double ry, double rz) {
 }
 
 // Kalman update with the measurement (ym, zm), plain gain form
-double kalman_update(const Config& cfg, Hyp& h, double ym, double zm) {
-    const Road rd = make_road(cfg, h);
+double kalman_update(const Config& cfg, Hyp& h, int layer, double ym, double zm) {
+    const Road rd = make_road(cfg, h, layer);
     const double r[2] = {ym - h.p[0], zm - h.p[1]};
     const double chi2inc = chi2_of(rd, r[0], r[1]);
     double K[5][2];
@@ -303,24 +330,25 @@ void find_candidates(const Config& cfg, const Store& st, const Hyp& h, int layer
     const std::vector<Tracklet>& v = st.cell[(size_t)h.sector * st.n_layers + layer];
     size_t lo = 0, hi = v.size();
     if (st.sorted) {
-        const double wide = rd.road_y * (1.0 + kLoose);
+        const double wide = (rd.road_y + std::fabs(rd.tan_tilt) * rd.road_z) * (1.0 + kLoose);
         lo = std::lower_bound(v.begin(), v.end(), h.p[0] - wide,
                               [](const Tracklet& a, double val) { return a.y < val; }) - v.begin();
         hi = std::upper_bound(v.begin(), v.end(), h.p[0] + wide,
                               [](double val, const Tracklet& a) { return val < a.y; }) - v.begin();
     }
-    const double veto = cfg.n_sigma_angle * cfg.sigma_dydx;
+    const double veto = rd.veto;
     for (size_t k = lo; k < hi; ++k) {
         const Tracklet& tl = v[k];
         if (cnt) cnt->n_scanned++;
         const double ry = tl.y - h.p[0], rz = tl.z - h.p[1];
+        const double ryc = ry - rd.tan_tilt * rz;                            // y corrected with the extrapolated z
         const double da = std::fabs(tl.dydx - rd.tanphi);
-        const bool in_y = std::fabs(ry) <= rd.road_y, in_z = std::fabs(rz) <= rd.road_z;
+        const bool in_y = std::fabs(ryc) <= rd.road_y, in_z = std::fabs(rz) <= rd.road_z;
         const bool pass = da <= veto;                                       // PAPER.md:60, 4 sigma [R8]
-        const bool loose_y = std::fabs(ry) <= rd.road_y * (1.0 + kLoose);
+        const bool loose_y = std::fabs(ryc) <= rd.road_y * (1.0 + kLoose);
         const bool loose_z = std::fabs(rz) <= rd.road_z * (1.0 + kLoose);
         const bool loose_a = da <= veto * (1.0 + kLoose);
-        if (loose_z && loose_a) note(margin, std::fabs(ry), rd.road_y);
+        if (loose_z && loose_a) note(margin, std::fabs(ryc), rd.road_y);
         if (loose_y && loose_a) note(margin, std::fabs(rz), rd.road_z);
         if (loose_y && loose_z) note(margin, da, veto);
         const double c2 = chi2_of(rd, ry, rz);                              // y and z only
@@ -362,7 +390,7 @@ void match_track(const Config& cfg, const Store& st, const Hyp& seed, TrackResul
             Hyp& h = prop[ih];
             if (h.alive) h.alive = propagate_to_layer(cfg, h, cfg.layer_x[L], mg, cnt);
             if (h.alive) {
-                const Road rd = make_road(cfg, h);
+                const Road rd = make_road(cfg, h, L);
                 if (cnt) cnt->n_road++;
                 find_candidates(cfg, st, h, L, rd, cands, &res.n_evals, mg, cnt);
                 for (const Cand& c : cands)
@@ -393,7 +421,7 @@ void match_track(const Config& cfg, const Store& st, const Hyp& seed, TrackResul
             Hyp h = prop[c.parent];
             h.score = c.score;
             if (c.tracklet != std::numeric_limits<int>::max()) {
-                const double chi2inc = kalman_update(cfg, h, c.y, c.z);
+                const double chi2inc = kalman_update(cfg, h, L, c.y, c.z);
                 if (cnt) cnt->n_upd++;
                 h.chi2 += chi2inc;
                 h.idx[L] = c.tracklet;
@@ -476,20 +504,20 @@ int orc_propagate_to_layer(const orc_config* cfg, double p[5], double c15[15], d
 }
 
 // Kalman update with (ym, zm); returns the chi2 increment
-double orc_update(const orc_config* cfg, double p[5], double c15[15], double ym, double zm) {
+double orc_update(const orc_config* cfg, double p[5], double c15[15], double ym, double zm, int layer) {
     Hyp h;
     load_hyp(h, p, c15, 0.0, 0);
-    const double c2 = kalman_update(*cfg, h, ym, zm);
+    const double c2 = kalman_update(*cfg, h, layer, ym, zm);
     std::memcpy(p, h.p, sizeof h.p);
     store_cov(h, c15);
     return c2;
 }
 
 // road half-widths and tan(phi) of a state: out = (road_y, road_z, tanphi, Sinv00, Sinv01, Sinv11)
-void orc_road(const orc_config* cfg, const double p[5], const double c15[15], double out[6]) {
+void orc_road(const orc_config* cfg, const double p[5], const double c15[15], double out[6], int layer) {
     Hyp h;
     load_hyp(h, p, c15, 0.0, 0);
-    const Road rd = make_road(*cfg, h);
+    const Road rd = make_road(*cfg, h, layer);
     out[0] = rd.road_y; out[1] = rd.road_z; out[2] = rd.tanphi;
     out[3] = rd.Sinv[0][0]; out[4] = rd.Sinv[0][1]; out[5] = rd.Sinv[1][1];
 }
@@ -502,7 +530,7 @@ int orc_candidates(const orc_config* cfg, const float* y, const float* z, const 
     build_store(*cfg, y, z, dydx, chamber, n, !brute, st);
     Hyp h;
     load_hyp(h, p, c15, cfg->layer_x[layer], sector);
-    const Road rd = make_road(*cfg, h);
+    const Road rd = make_road(*cfg, h, layer);
     std::vector<Cand> cands;
     find_candidates(*cfg, st, h, layer, rd, cands, nullptr, nullptr, nullptr);
     std::sort(cands.begin(), cands.end(), [](const Cand& a, const Cand& b) { return a.index < b.index; });

@@ -54,6 +54,13 @@ EFFICIENCY = 0.9
 MAX_SNP = 0.95
 NOISE_DYDX_RANGE = 0.5
 
+# Resolution model of PAPER.md:62 / Fig. 3 (image not available: the coefficients below are this build's synthetic
+# choice, R24) and pad tilt of PAPER.md:66 (R25).  sigma(s) = c0 + c2 (s - sin(Lorentz angle))^2.
+SY_C0, SY_C2 = 0.03, 0.12            # cm: 0.03 at the optimum, 0.06 at |s - sL| = 0.5
+SD_C0, SD_C2 = 0.015, 0.06           # dy/dx: "below 1 degree" at the optimum
+LORENTZ_DEG = 8.0
+TILT_DEG = 2.0
+
 
 @dataclasses.dataclass(frozen=True)
 class WorkloadSpec:
@@ -72,6 +79,7 @@ class WorkloadSpec:
     smear_tracklets: bool = True
     exact_z: bool = False             # tracklet z = true z instead of the pad-row centre
     efficiency: float = EFFICIENCY
+    res_model: int = 0                # 1: sigma_y(sin phi), sigma_dydx(sin phi) polynomials and +-2 degree pad tilt
 
     @property
     def seed(self) -> int:
@@ -95,12 +103,21 @@ def scaled(spec: WorkloadSpec, n_tracks: int, name: Optional[str] = None) -> Wor
                                batch=None if spec.batch is None else min(spec.batch, n_tracks))
 
 
+def sin_lorentz(bz: float) -> float:
+    """sin of the Lorentz angle; its sign follows the field polarity ("+-8 degrees")."""
+    return math.copysign(math.sin(math.radians(LORENTZ_DEG)), bz) if bz != 0.0 else 0.0
+
+
 def matcher_config(spec: WorkloadSpec) -> dict:
     """The cuts and geometry of a config as a plain dict (field names of include/trdmatch.h).
 
     Both the oracle wrapper and the CUDA binding turn this dict into their own struct.
     """
-    return dict(
+    extra = {}
+    if spec.res_model:
+        extra = dict(res_model=1, sy_c0=SY_C0, sy_c2=SY_C2, sd_c0=SD_C0, sd_c2=SD_C2,
+                     sin_lorentz=sin_lorentz(spec.bz), tan_tilt=math.tan(math.radians(TILT_DEG)))
+    return dict(extra, 
         n_sectors=N_SECTORS, n_stacks=N_STACKS, n_layers=N_LAYERS,
         layer_x=list(LAYER_X), z_max=Z_MAX, pad_length=PAD_LENGTH, bz_tesla=spec.bz,
         sigma_y=SIGMA_Y_TRACKLET, sigma_z=PAD_LENGTH / math.sqrt(12.0),
@@ -240,11 +257,20 @@ def generate(spec: WorkloadSpec) -> dict:
         if lay == N_LAYERS - 1:
             truth_last[okl] = np.stack([yl, zl, sl, secl.astype(float)], axis=1)[okl]
         idx = np.nonzero(present)[0]
-        yy = yl[idx] + (SIGMA_Y_TRACKLET * ny[idx] if spec.smear_tracklets else 0.0)
         zc = pad_row_centre(zl[idx])
         zz = zl[idx] if spec.exact_z else zc
         tanphi = sl[idx] / np.sqrt(1.0 - sl[idx] ** 2)
-        dd = tanphi + (SIGMA_DYDX_TRACKLET * nd[idx] if spec.smear_tracklets else 0.0)
+        if spec.res_model:
+            # precise coordinate across the tilted pad, coarse one along it: the z error (row centre instead of
+            # the true z) leaks into y with tan(tilt); resolutions depend on the true sin(phi)
+            ds = sl[idx] - sin_lorentz(spec.bz)
+            sig_y_l, sig_d_l = SY_C0 + SY_C2 * ds * ds, SD_C0 + SD_C2 * ds * ds
+            tilt = math.radians(TILT_DEG) * (1.0 if lay % 2 == 0 else -1.0)
+            yy = yl[idx] + math.tan(tilt) * (zz - zl[idx]) + (math.cos(tilt) * sig_y_l * ny[idx] if spec.smear_tracklets else 0.0)
+            dd = tanphi + (sig_d_l * nd[idx] if spec.smear_tracklets else 0.0)
+        else:
+            yy = yl[idx] + (SIGMA_Y_TRACKLET * ny[idx] if spec.smear_tracklets else 0.0)
+            dd = tanphi + (SIGMA_DYDX_TRACKLET * nd[idx] if spec.smear_tracklets else 0.0)
         sig_y.append(yy); sig_z.append(zz); sig_d.append(dd)
         sig_ch.append(secl[idx] * (N_STACKS * N_LAYERS) + stack_of_z(zc) * N_LAYERS + lay)
         sig_lab.append(idx); sig_lay.append(np.full(idx.shape[0], lay))
