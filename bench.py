@@ -329,11 +329,16 @@ def main():
     ap.add_argument("--workload", default="timeframe")
     ap.add_argument("--tracks", type=int, default=0, help="scale the workload to this many tracks (debugging)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--res-model", type=int, default=0, choices=[0, 1],
+                    help="1: inputs and matcher with the sin(phi)-dependent resolutions and pad tilt (SURVEY.md 8(f) NEXT#1)")
     args = ap.parse_args()
     from paper_2003_03174_b200 import workloads as W
     spec = W.CONFIGS[args.workload]
     if args.tracks:
         spec = W.scaled(spec, args.tracks)
+    if args.res_model:
+        import dataclasses
+        spec = dataclasses.replace(spec, res_model=1, name=spec.name + "_res1")
     cfg = W.matcher_config(spec)
     if args.impl == "reference":
         run_reference(args, spec, cfg)

@@ -73,7 +73,16 @@ typedef struct trd_config {
                                         before matching, for cache locality: 0 = when it pays (large batch
                                         against a large index), 1 = always, -1 = never.  Results do not
                                         depend on it. */
-    int32_t reserved_;               /* 0 */
+    int32_t res_model;               /* measurement model.  0: constant sigma_y, sigma_dydx, no pad tilt (the configs).
+                                        1 (Fig. 3): sigma_y and sigma_dydx are second-order
+                                        polynomials of the track's sin(phi), c0 + c2 (sin(phi) - sin_lorentz)^2, and the
+                                        pads of layer l are tilted by +tilt (l even) / -tilt (l odd): tracklet covariance
+                                        R = Rot(tau) diag(sigma_y^2, sigma_z^2) Rot(tau)^T, y road on the residual corrected
+                                        with the extrapolated z, r_y - tan(tau) r_z */
+    double sy_c0, sy_c2;             /* sigma_y(s)    [cm]    (res_model = 1) */
+    double sd_c0, sd_c2;             /* sigma_dydx(s)         (res_model = 1) */
+    double sin_lorentz;              /* optimum of both polynomials, sin of the Lorentz angle (about +-8 degrees) */
+    double tan_tilt;                 /* tan of the pad tilt (2 degrees) */
 } trd_config;
 
 /* Input tracks of one batch: device pointers, each of length n_tracks. */

@@ -35,7 +35,9 @@ class TrdConfig(C.Structure):
                 ("sigma_y", C.c_double), ("sigma_z", C.c_double), ("sigma_dydx", C.c_double),
                 ("n_sigma_road", C.c_double), ("n_sigma_angle", C.c_double), ("chi2_cut", C.c_double),
                 ("chi2_penalty", C.c_double), ("max_snp", C.c_double), ("ybin_width", C.c_double),
-                ("track_binning", C.c_int32), ("reserved_", C.c_int32)]
+                ("track_binning", C.c_int32), ("res_model", C.c_int32),
+                ("sy_c0", C.c_double), ("sy_c2", C.c_double), ("sd_c0", C.c_double), ("sd_c2", C.c_double),
+                ("sin_lorentz", C.c_double), ("tan_tilt", C.c_double)]
 
 
 class TrdTracksIn(C.Structure):
@@ -110,6 +112,9 @@ def make_config(cfg: dict) -> TrdConfig:
         setattr(c, k, float(cfg[k]))
     c.ybin_width = float(cfg.get("ybin_width", 0.0))
     c.track_binning = int(cfg.get("track_binning", 0))
+    c.res_model = int(cfg.get("res_model", 0))
+    for k in ("sy_c0", "sy_c2", "sd_c0", "sd_c2", "sin_lorentz", "tan_tilt"):
+        setattr(c, k, float(cfg.get(k, 0.0)))
     return c
 
 

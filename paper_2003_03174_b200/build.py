@@ -19,7 +19,7 @@ LIB_DIR = os.path.join(_HERE, "lib")
 LIB_PATH = os.path.join(LIB_DIR, "libtrdmatch.so")
 SOURCES = ("api.cu", "host_api.cu", "index.cu", "match.cu", "tracks.cu")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-              "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"]
+              "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr", "-fmad=false"]
 
 
 def _nvcc() -> str:

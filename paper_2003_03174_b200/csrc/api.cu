@@ -55,6 +55,14 @@ bool derive_params(const trd_config& c, trd::MatchParams& mp) {
     mp.chi2_cut = (float)c.chi2_cut;
     mp.chi2_penalty = (float)c.chi2_penalty;
     mp.max_snp = (float)c.max_snp;
+    mp.res_model = c.res_model;
+    mp.n_sigma_angle = (float)c.n_sigma_angle;
+    mp.sy_c0 = (float)c.sy_c0;
+    mp.sy_c2 = (float)c.sy_c2;
+    mp.sd_c0 = (float)c.sd_c0;
+    mp.sd_c2 = (float)c.sd_c2;
+    mp.sin_lorentz = (float)c.sin_lorentz;
+    mp.tan_tilt = (float)c.tan_tilt;
     return true;
 }
 
@@ -77,6 +85,11 @@ const char* check_config(const trd_config& c) {
     if (!(c.max_snp > 0.0) || !(c.max_snp < 1.0)) return "max_snp must be in (0, 1)";
     if (!(c.ybin_width >= 0.0)) return "ybin_width must be >= 0";
     if (c.track_binning < -1 || c.track_binning > 1) return "track_binning must be -1, 0 or 1";
+    if (c.res_model != 0 && c.res_model != 1) return "res_model must be 0 or 1";
+    if (c.res_model == 1) {
+        if (!(c.sy_c0 > 0.0) || !(c.sd_c0 > 0.0) || !(c.sy_c2 >= 0.0) || !(c.sd_c2 >= 0.0)) return "resolution coefficients out of range";
+        if (!(fabs(c.sin_lorentz) < 1.0) || !(fabs(c.tan_tilt) < 1.0)) return "sin_lorentz / tan_tilt out of range";
+    }
     return nullptr;
 }
 

@@ -46,6 +46,9 @@ struct MatchParams {
     float n_sigma_road, half_pad;
     float veto;                      // n_sigma_angle * sigma_dydx
     float chi2_cut, chi2_penalty, max_snp;
+    // measurement model (res_model = 1: PAPER.md:62, 66)
+    int res_model;
+    float n_sigma_angle, sy_c0, sy_c2, sd_c0, sd_c2, sin_lorentz, tan_tilt;
 };
 
 struct Buffer {

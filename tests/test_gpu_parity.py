@@ -245,3 +245,27 @@ def test_pipelined_host_entry_points(B):
                 np.testing.assert_array_equal(got, want[k])
     finally:
         B.trd_destroy(h)
+
+
+@pytest.mark.parametrize("name,n_hyp", [("central", 1), ("central8", 8), ("pileup", 4)])
+def test_resolution_model_and_pad_tilt(B, name, n_hyp):
+    """sigma_y(sin phi), sigma_dydx(sin phi) and the +-2 degree pad tilt
+    (res_model = 1), inputs generated with the same model; same parity criteria as the configs."""
+    spec = dataclasses.replace(W.CONFIGS[name], res_model=1, n_hyp=n_hyp)
+    d = W.generate(spec); cfg = W.matcher_config(spec)
+    assert cfg["res_model"] == 1 and cfg["tan_tilt"] > 0.03
+    want = O.match(cfg, d)
+    assert_parity(P.compare(run_gpu(B, cfg, d), want), want)
+    assert_parity(P.compare(run_gpu(B, dict(cfg, track_binning=1), d, batch=1777), want), want)
+    # the model matters: the same input matched without the tilt loses tracklets
+    plain = run_gpu(B, dict(cfg, tan_tilt=0.0), d)
+    assert plain["n_matched"].sum() < 0.97 * want["n_matched"].sum()
+
+
+def test_resolution_model_dense(B):
+    spec = dataclasses.replace(W.CONFIGS["tiny"], name="dense", number=8, n_tracks=3000, n_noise=12_000_000, n_hyp=4,
+                               res_model=1)
+    d = W.generate(spec); cfg = W.matcher_config(spec)
+    want = O.match(cfg, d)
+    assert want["counters"]["n_cand"] > want["counters"]["n_road"]
+    assert_parity(P.compare(run_gpu(B, cfg, d), want), want)
