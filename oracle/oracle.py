@@ -163,11 +163,19 @@ def match(cfg: dict, data: dict, brute: bool = False, n_threads: int = 0, lo: in
                sector=np.zeros(n, np.int32), chi2=np.zeros(n), n_matched=np.zeros(n, np.int32),
                n_evals=np.zeros(n, np.int32), margin=np.zeros(n))
     counters = np.zeros(6, np.int64); seconds = np.zeros(2)
+    # time-frame association: interaction ids of tracklets and tracks, if the inputs carry them
+    n_ia = int(data.get("n_interactions", 0) or 0)
+    if n_ia > 1:
+        tl_ia = np.ascontiguousarray(data["tl_interaction"]); trk_ia = np.ascontiguousarray(data["interaction"][lo:hi])
+        assert tl_ia.dtype == np.int32 and trk_ia.dtype == np.int32
+        ia_args = (_ip(tl_ia), _ip(trk_ia), n_ia)
+    else:
+        ia_args = (None, None, 1)
     rc = lib().orc_match(C.byref(make_config(cfg)), _fp(y), _fp(z), _fp(d), _ip(ch), C.c_int64(y.shape[0]),
                          _fp(par), _fp(cov), _fp(x), _ip(sec), C.c_int64(n), int(brute), int(n_threads),
                          _ip(out["idx"]), _dp(out["par"]), _dp(out["cov"]), _dp(out["x"]), _ip(out["sector"]),
                          _dp(out["chi2"]), _ip(out["n_matched"]), _ip(out["n_evals"]), _dp(out["margin"]),
-                         counters.ctypes.data_as(C.POINTER(C.c_int64)), _dp(seconds))
+                         counters.ctypes.data_as(C.POINTER(C.c_int64)), _dp(seconds), *ia_args)
     if rc != 0:
         raise RuntimeError(f"orc_match failed: {rc}")
     out["counters"] = dict(zip(("n_prop", "n_rot", "n_road", "n_cand", "n_upd", "n_scanned"), counters.tolist()))

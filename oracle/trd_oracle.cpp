@@ -65,11 +65,13 @@ struct Hyp {
     int idx[kMaxLayers];
     int n_matched;
     bool alive;
+    int ia;            // interaction of the track [R27]
 };
 
 struct Tracklet {
     double y, z, dydx;
     int index;         // position in the caller's arrays
+    int ia;            // interaction (collision) the tracklet belongs to; 0 without time-frame association [R27]
 };
 
 struct Counters {
@@ -290,24 +292,33 @@ double kalman_update(const Config& cfg, Hyp& h, int layer, double ym, double zm)
 }
 
 // ---- tracklet store: one list per (sector, layer), sorted by y --------------------------
+// Time-frame association ("only those tracklets which belong to the same interaction") [R27]:
+// with n_ia > 1 every tracklet and track carries an interaction id in 0..n_ia-1 and only equal ids match.  The
+// sorted store keeps one y-sorted list per (interaction, sector, layer); the brute-force store keeps one list
+// per (sector, layer) and compares the ids tracklet by tracklet -- the two must give identical results.
 struct Store {
-    int n_sectors = 0, n_layers = 0;
-    std::vector<std::vector<Tracklet>> cell;   // [sector * n_layers + layer]
-    bool sorted = false;
+    int n_sectors = 0, n_layers = 0, n_ia = 1;
+    std::vector<std::vector<Tracklet>> cell;   // [(ia *) sector * n_layers + layer]
+    bool sorted = false, by_ia = false;
 };
 
 void build_store(const Config& cfg, const float* y, const float* z, const float* dydx, const int32_t* chamber,
-                 int64_t n, bool sort_by_y, Store& st) {
+                 const int32_t* ia, int n_ia, int64_t n, bool sort_by_y, Store& st) {
     st.n_sectors = cfg.n_sectors;
     st.n_layers = cfg.n_layers;
-    st.cell.assign((size_t)cfg.n_sectors * cfg.n_layers, {});
+    st.n_ia = (ia && n_ia > 1) ? n_ia : 1;
+    st.by_ia = sort_by_y && st.n_ia > 1;
+    st.cell.assign((size_t)(st.by_ia ? st.n_ia : 1) * cfg.n_sectors * cfg.n_layers, {});
     const int per_sector = cfg.n_stacks * cfg.n_layers;
     for (int64_t i = 0; i < n; ++i) {
         const int ch = chamber[i];
         if (ch < 0 || ch >= cfg.n_sectors * per_sector) continue;             // unusable tracklet
         if (!std::isfinite(y[i]) || !std::isfinite(z[i])) continue;
+        const int a = (st.n_ia > 1) ? ia[i] : 0;
+        if (a < 0 || a >= st.n_ia) continue;                                  // no such interaction
         const int sector = ch / per_sector, layer = ch % cfg.n_layers;        // stack id unused [R12]
-        st.cell[(size_t)sector * cfg.n_layers + layer].push_back({(double)y[i], (double)z[i], (double)dydx[i], (int)i});
+        const size_t c = ((size_t)(st.by_ia ? a : 0) * cfg.n_sectors + sector) * cfg.n_layers + layer;
+        st.cell[c].push_back({(double)y[i], (double)z[i], (double)dydx[i], (int)i, a});
     }
     if (sort_by_y)
         for (auto& v : st.cell)
@@ -327,7 +338,8 @@ struct Cand {
 void find_candidates(const Config& cfg, const Store& st, const Hyp& h, int layer, const Road& rd,
                      std::vector<Cand>& out, int* n_evals, double* margin, Counters* cnt) {
     out.clear();
-    const std::vector<Tracklet>& v = st.cell[(size_t)h.sector * st.n_layers + layer];
+    if (st.n_ia > 1 && (h.ia < 0 || h.ia >= st.n_ia)) return;                // a track of no known interaction
+    const std::vector<Tracklet>& v = st.cell[((size_t)(st.by_ia ? h.ia : 0) * st.n_sectors + h.sector) * st.n_layers + layer];
     size_t lo = 0, hi = v.size();
     if (st.sorted) {
         const double wide = (rd.road_y + std::fabs(rd.tan_tilt) * rd.road_z) * (1.0 + kLoose);
@@ -339,6 +351,7 @@ void find_candidates(const Config& cfg, const Store& st, const Hyp& h, int layer
     const double veto = rd.veto;
     for (size_t k = lo; k < hi; ++k) {
         const Tracklet& tl = v[k];
+        if (tl.ia != h.ia) continue;                                         // other interaction [R27]
         if (cnt) cnt->n_scanned++;
         const double ry = tl.y - h.p[0], rz = tl.z - h.p[1];
         const double ryc = ry - rd.tan_tilt * rz;                            // y corrected with the extrapolated z
@@ -527,7 +540,7 @@ int orc_candidates(const orc_config* cfg, const float* y, const float* z, const 
                    int64_t n, const double p[5], const double c15[15], int sector, int layer, int brute,
                    int32_t* out_index, double* out_chi2, int cap) {
     Store st;
-    build_store(*cfg, y, z, dydx, chamber, n, !brute, st);
+    build_store(*cfg, y, z, dydx, chamber, nullptr, 1, n, !brute, st);
     Hyp h;
     load_hyp(h, p, c15, cfg->layer_x[layer], sector);
     const Road rd = make_road(*cfg, h, layer);
@@ -550,11 +563,13 @@ int orc_match(const orc_config* cfg, const float* tl_y, const float* tl_z, const
               const int32_t* tl_chamber, int64_t n_tl, const float* par, const float* cov, const float* x,
               const int32_t* sector, int64_t n_trk, int brute, int n_threads, int32_t* out_idx, double* out_par,
               double* out_cov, double* out_x, int32_t* out_sector, double* out_chi2, int32_t* out_n_matched,
-              int32_t* out_n_evals, double* out_margin, int64_t counters[6], double seconds[2]) {
+              int32_t* out_n_evals, double* out_margin, int64_t counters[6], double seconds[2],
+              const int32_t* tl_ia, const int32_t* trk_ia, int32_t n_ia) {
     if (cfg->n_layers > kMaxLayers || cfg->n_hyp < 1) return -1;
+    if ((tl_ia == nullptr) != (trk_ia == nullptr)) return -2;
     const auto t0 = std::chrono::steady_clock::now();
     Store st;
-    build_store(*cfg, tl_y, tl_z, tl_dydx, tl_chamber, n_tl, !brute, st);
+    build_store(*cfg, tl_y, tl_z, tl_dydx, tl_chamber, tl_ia, n_ia, n_tl, !brute, st);
     const auto t1 = std::chrono::steady_clock::now();
     Counters total;
 #ifdef _OPENMP
@@ -570,6 +585,7 @@ int orc_match(const orc_config* cfg, const float* tl_y, const float* tl_z, const
             for (int k = 0; k < 15; ++k) c15[k] = cov[k * n_trk + i];
             Hyp seed;
             load_hyp(seed, p, c15, x[i], sector[i]);
+            seed.ia = (st.n_ia > 1) ? trk_ia[i] : 0;
             seed.alive = std::fabs(p[2]) < cfg->max_snp && sector[i] >= 0 && sector[i] < cfg->n_sectors;
             TrackResult res;
             match_track(*cfg, st, seed, res, &local);

@@ -80,6 +80,8 @@ class WorkloadSpec:
     exact_z: bool = False             # tracklet z = true z instead of the pad-row centre
     efficiency: float = EFFICIENCY
     res_model: int = 0                # 1: sigma_y(sin phi), sigma_dydx(sin phi) polynomials and +-2 degree pad tilt
+    n_interactions: int = 0           # > 1: time-frame association: tracks i*n_ia//n_tracks form one
+                                      # collision, their tracklets inherit its id, noise tracklets get a random one
 
     @property
     def seed(self) -> int:
@@ -289,6 +291,10 @@ def generate(spec: WorkloadSpec) -> dict:
         sel = st_n == k
         z_n[sel] = rows[k][np.minimum((pick[sel] * len(rows[k])).astype(np.int64), len(rows[k]) - 1)]
     d_n = rng.uniform(-NOISE_DYDX_RANGE, NOISE_DYDX_RANGE, m_noise)
+    n_ia = spec.n_interactions if spec.n_interactions > 1 else 0
+    if n_ia:                                               # drawn only for associated specs: other specs' bytes unchanged
+        trk_ia = (np.arange(n, dtype=np.int64) * n_ia) // n
+        ia_n = rng.integers(0, n_ia, m_noise)
 
     # 5. concatenate and permute
     tl_y = np.concatenate(sig_y + [y_n]); tl_z = np.concatenate(sig_z + [z_n])
@@ -298,12 +304,16 @@ def generate(spec: WorkloadSpec) -> dict:
     m = tl_y.shape[0]
     perm = rng.permutation(m)
     tl_y, tl_z, tl_d, tl_ch, tl_lab, tl_lay = (a[perm] for a in (tl_y, tl_z, tl_d, tl_ch, tl_lab, tl_lay))
+    assoc = {}
+    if n_ia:
+        tl_ia = np.concatenate([trk_ia[i] for i in sig_lab] + [ia_n])[perm]
+        assoc = dict(n_interactions=n_ia, interaction=trk_ia.astype(np.int32), tl_interaction=tl_ia.astype(np.int32))
     truth_idx = np.full((n, N_LAYERS), -1, np.int32)
     is_sig = tl_lab >= 0
     truth_idx[tl_lab[is_sig], tl_lay[is_sig]] = np.nonzero(is_sig)[0].astype(np.int32)
 
     return dict(
-        spec=spec,
+        assoc, spec=spec,
         par=np.ascontiguousarray(par, np.float32), cov=np.ascontiguousarray(cov, np.float32),
         x=np.full(n, X_SEED, np.float32), sector=sec.astype(np.int32),
         tl_y=tl_y.astype(np.float32), tl_z=tl_z.astype(np.float32), tl_dydx=tl_d.astype(np.float32),
