@@ -91,6 +91,8 @@ typedef struct trd_tracks_in {
     const float* cov[15];   /* lower triangle, order above */
     const float* x;         /* local x of the state (247 in the configs) */
     const int32_t* sector;  /* sector frame of the state, 0..n_sectors-1 */
+    const int32_t* interaction; /* interaction (collision) of the track, 0..n_interactions-1; read only when the
+                                   index was built by trd_load_tracklets_tf with n_interactions > 1, else may be NULL */
 } trd_tracks_in;
 
 /* Output of one batch: caller-allocated device pointers, each of length n_tracks.  The best
@@ -120,6 +122,8 @@ typedef struct trd_index_info {
     double ybin_width;     /* cm */
     int32_t key_bits;      /* radix-sorted key width */
     int32_t n_passes;      /* 8-bit radix passes */
+    int32_t n_interactions; /* 1 = no time-frame association */
+    int32_t reserved_;
 } trd_index_info;
 
 typedef struct trd_handle trd_handle;
@@ -142,6 +146,16 @@ void trd_destroy(trd_handle* h);
  * `stream` by this call has run. */
 int trd_load_tracklets(trd_handle* h, const float* d_y, const float* d_z, const float* d_dydx,
                        const int32_t* d_chamber, int64_t n, void* stream);
+
+/* Time-frame variant (tracklets are matched only to tracks of the same interaction): as
+ * trd_load_tracklets, with the interaction id of every tracklet (device array, 0..n_interactions-1; other values
+ * make the tracklet unusable).  The id leads the bin key, so a track only ever scans tracklets of its own
+ * interaction.  trd_match then reads trd_tracks_in.interaction; a track whose id is out of range is propagated
+ * but attaches nothing.  n_interactions <= 1 or d_interaction == NULL is trd_load_tracklets.  Device arrays only
+ * (the *_host entry points do not carry interaction ids in this version). */
+int trd_load_tracklets_tf(trd_handle* h, const float* d_y, const float* d_z, const float* d_dydx,
+                          const int32_t* d_chamber, const int32_t* d_interaction, int32_t n_interactions, int64_t n,
+                          void* stream);
 
 /* The tracking step for one batch (n_tracks >= 0) against the loaded index. */
 int trd_match(trd_handle* h, const trd_tracks_in* in, const trd_tracks_out* out, int64_t n_tracks,

@@ -20,7 +20,7 @@ TRD_MAX_HYP = 8
 TRD_OK, TRD_E_ARG, TRD_E_CUDA, TRD_E_NOMEM, TRD_E_STATE = 0, -1, -2, -3, -4
 _STATUS = {0: "TRD_OK", -1: "TRD_E_ARG", -2: "TRD_E_CUDA", -3: "TRD_E_NOMEM", -4: "TRD_E_STATE"}
 
-EXPORTS = ("trd_version", "trd_create", "trd_destroy", "trd_load_tracklets", "trd_match",
+EXPORTS = ("trd_version", "trd_create", "trd_destroy", "trd_load_tracklets", "trd_load_tracklets_tf", "trd_match",
            "trd_load_tracklets_host", "trd_match_host", "trd_match_host_async", "trd_wait_host", "trd_get_index_info", "trd_copy_index",
            "trd_last_error", "trd_device_bytes", "trd_kernel_launches", "trd_last_match_kernel_ms")
 
@@ -41,7 +41,8 @@ class TrdConfig(C.Structure):
 
 
 class TrdTracksIn(C.Structure):
-    _fields_ = [("par", C.c_void_p * 5), ("cov", C.c_void_p * 15), ("x", C.c_void_p), ("sector", C.c_void_p)]
+    _fields_ = [("par", C.c_void_p * 5), ("cov", C.c_void_p * 15), ("x", C.c_void_p), ("sector", C.c_void_p),
+                ("interaction", C.c_void_p)]
 
 
 class TrdTracksOut(C.Structure):
@@ -52,7 +53,8 @@ class TrdTracksOut(C.Structure):
 
 class TrdIndexInfo(C.Structure):
     _fields_ = [("n_tracklets", C.c_int64), ("n_zrows", C.c_int32), ("n_ybins", C.c_int32), ("n_bins", C.c_int64),
-                ("ybin_width", C.c_double), ("key_bits", C.c_int32), ("n_passes", C.c_int32)]
+                ("ybin_width", C.c_double), ("key_bits", C.c_int32), ("n_passes", C.c_int32),
+                ("n_interactions", C.c_int32), ("reserved_", C.c_int32)]
 
 
 class TrdError(RuntimeError):
@@ -83,6 +85,8 @@ def lib():
         l.trd_destroy.restype = None
         l.trd_load_tracklets.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p]
         l.trd_load_tracklets_host.argtypes = l.trd_load_tracklets.argtypes
+        l.trd_load_tracklets_tf.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32,
+                                            C.c_int64, C.c_void_p]
         l.trd_match.argtypes = [C.c_void_p, C.POINTER(TrdTracksIn), C.POINTER(TrdTracksOut), C.c_int64, C.c_void_p]
         l.trd_match_host.argtypes = l.trd_match.argtypes
         l.trd_match_host_async.argtypes = l.trd_match.argtypes
@@ -165,6 +169,15 @@ def trd_load_tracklets(h, d_y, d_z, d_dydx, d_chamber, n: Optional[int] = None, 
                                        _dev_ptr(d_chamber, "i32", n), n, _stream(stream)))
 
 
+def trd_load_tracklets_tf(h, d_y, d_z, d_dydx, d_chamber, d_interaction, n_interactions: int, n: Optional[int] = None,
+                          stream=None) -> None:
+    """Time-frame variant: tracklets carry interaction ids (int32 CUDA tensor); see include/trdmatch.h."""
+    n = d_y.numel() if n is None else n
+    _check(h, lib().trd_load_tracklets_tf(h, _dev_ptr(d_y, "f32", n), _dev_ptr(d_z, "f32", n), _dev_ptr(d_dydx, "f32", n),
+                                          _dev_ptr(d_chamber, "i32", n), _dev_ptr(d_interaction, "i32", n),
+                                          int(n_interactions), n, _stream(stream)))
+
+
 def alloc_tracks_out(n: int, device="cuda", with_evals: bool = True) -> Dict[str, "object"]:
     import torch
     out = dict(idx=torch.empty((TRD_MAX_LAYERS, n), dtype=torch.int32, device=device),
@@ -197,6 +210,7 @@ def trd_match(h, tracks: dict, out: Optional[dict] = None, n_tracks: Optional[in
         tin.cov[:] = _row_ptrs(tracks["cov"], 15, n, "f32")
         tin.x = _dev_ptr(tracks["x"], "f32", n)
         tin.sector = _dev_ptr(tracks["sector"], "i32", n)
+        tin.interaction = _dev_ptr(tracks["interaction"], "i32", n) if "interaction" in tracks else None
         tout.tracklet_idx[:] = _row_ptrs(out["idx"], TRD_MAX_LAYERS, n, "i32")
         tout.par[:] = _row_ptrs(out["par"], 5, n, "f32")
         tout.cov[:] = _row_ptrs(out["cov"], 15, n, "f32")
@@ -307,8 +321,8 @@ def trd_last_match_kernel_ms(h) -> float:
 def to_device(data: dict, device="cuda") -> dict:
     """Upload the arrays of workloads.generate as torch tensors (tracks and tracklets)."""
     import torch
-    keys = ("par", "cov", "x", "sector", "tl_y", "tl_z", "tl_dydx", "tl_chamber")
-    return {k: torch.from_numpy(np.ascontiguousarray(data[k])).to(device) for k in keys}
+    keys = ("par", "cov", "x", "sector", "tl_y", "tl_z", "tl_dydx", "tl_chamber", "interaction", "tl_interaction")
+    return {k: torch.from_numpy(np.ascontiguousarray(data[k])).to(device) for k in keys if k in data}
 
 
 def to_numpy(out: dict) -> dict:

@@ -158,8 +158,21 @@ int trd_load_tracklets(trd_handle* h, const float* d_y, const float* d_z, const 
     if (!h) return TRD_E_ARG;
     if (n < 0 || n >= (1 << 29) - 1) return fail(h, TRD_E_ARG, "trd_load_tracklets: n out of range (must be < 2^29 - 1)");
     if (n > 0 && (!d_y || !d_z || !d_dydx || !d_chamber)) return fail(h, TRD_E_ARG, "trd_load_tracklets: NULL array");
-    const cudaError_t e = trd::build_index(h, d_y, d_z, d_dydx, d_chamber, n, (cudaStream_t)stream);
+    const cudaError_t e = trd::build_index(h, d_y, d_z, d_dydx, d_chamber, nullptr, 1, n, (cudaStream_t)stream);
     if (e != cudaSuccess) return fail_cuda(h, e, "trd_load_tracklets");
+    return TRD_OK;
+}
+
+int trd_load_tracklets_tf(trd_handle* h, const float* d_y, const float* d_z, const float* d_dydx,
+                          const int32_t* d_chamber, const int32_t* d_interaction, int32_t n_interactions, int64_t n,
+                          void* stream) {
+    if (!h) return TRD_E_ARG;
+    if (n < 0 || n >= (1 << 29) - 1) return fail(h, TRD_E_ARG, "trd_load_tracklets_tf: n out of range (must be < 2^29 - 1)");
+    if (n > 0 && (!d_y || !d_z || !d_dydx || !d_chamber)) return fail(h, TRD_E_ARG, "trd_load_tracklets_tf: NULL array");
+    if (n_interactions > (1 << 20)) return fail(h, TRD_E_ARG, "trd_load_tracklets_tf: too many interactions");
+    const cudaError_t e = trd::build_index(h, d_y, d_z, d_dydx, d_chamber, d_interaction, n_interactions, n, (cudaStream_t)stream);
+    if (e == cudaErrorInvalidValue) return fail(h, TRD_E_ARG, "trd_load_tracklets_tf: interactions x rows exceed the key range");
+    if (e != cudaSuccess) return fail_cuda(h, e, "trd_load_tracklets_tf");
     return TRD_OK;
 }
 
@@ -176,6 +189,8 @@ int trd_match(trd_handle* h, const trd_tracks_in* in, const trd_tracks_out* out,
         if (!out->tracklet_idx[l]) return fail(h, TRD_E_ARG, "trd_match: NULL tracklet_idx array");
     if (!in->x || !in->sector || !out->x || !out->sector || !out->chi2 || !out->n_matched)
         return fail(h, TRD_E_ARG, "trd_match: NULL array");
+    if (h->mp.g.n_ia > 1 && !in->interaction)
+        return fail(h, TRD_E_ARG, "trd_match: the index carries interactions but trd_tracks_in.interaction is NULL");
     const cudaError_t e = trd::launch_match(h, *in, *out, n_tracks, (cudaStream_t)stream);
     if (e != cudaSuccess) return fail_cuda(h, e, "trd_match");
     return TRD_OK;
@@ -191,6 +206,8 @@ int trd_get_index_info(const trd_handle* h, trd_index_info* info) {
     info->ybin_width = h->ybin_width;
     info->key_bits = h->key_bits;
     info->n_passes = h->n_passes;
+    info->n_interactions = h->mp.g.n_ia;
+    info->reserved_ = 0;
     return TRD_OK;
 }
 

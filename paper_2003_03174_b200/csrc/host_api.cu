@@ -61,7 +61,7 @@ cudaError_t load_host(trd_handle* h, const float* y, const float* z, const float
     TRD_TRY(cudaEventRecord(h->ev_tl_in, h->s_in));
     TRD_TRY(cudaStreamWaitEvent(st, h->ev_tl_in, 0));
     TRD_TRY(build_index(h, (const float*)base, (const float*)(base + bytes), (const float*)(base + 2 * bytes),
-                        (const int32_t*)(base + 3 * bytes), n, st));
+                        (const int32_t*)(base + 3 * bytes), nullptr, 1, n, st));
     TRD_TRY(cudaEventRecord(h->ev_tl_used, st));
     h->tl_pending = true;
     return cudaSuccess;
@@ -86,6 +86,7 @@ cudaError_t match_host_async(trd_handle* h, const trd_tracks_in& in, const trd_t
     for (int j = 0; j < 15; ++j) { src[a] = in.cov[j]; din.cov[j] = (const float*)(bi + a * bytes); ++a; }
     src[a] = in.x; din.x = (const float*)(bi + a * bytes); ++a;
     src[a] = in.sector; din.sector = (const int32_t*)(bi + a * bytes); ++a;
+    din.interaction = nullptr;
     int b = 0;
     for (int l = 0; l < TRD_MAX_LAYERS; ++l) { dst[b] = out.tracklet_idx[l]; dout.tracklet_idx[l] = (int32_t*)(bo + b * bytes); ++b; }
     for (int j = 0; j < 5; ++j) { dst[b] = out.par[j]; dout.par[j] = (float*)(bo + b * bytes); ++b; }
@@ -155,6 +156,7 @@ int trd_match_host_async(trd_handle* h, const trd_tracks_in* in, const trd_track
     if (!h) return TRD_E_ARG;
     if (!in || !out || n < 0) return trd::fail(h, TRD_E_ARG, "trd_match_host: NULL struct or negative n_tracks");
     if (!h->index_loaded) return trd::fail(h, TRD_E_STATE, "trd_match_host: no tracklets loaded");
+    if (h->mp.g.n_ia > 1) return trd::fail(h, TRD_E_STATE, "trd_match_host: the index carries interactions; use trd_match");
     if (n == 0) return TRD_OK;
     for (int k = 0; k < 5; ++k)
         if (!in->par[k] || !out->par[k]) return trd::fail(h, TRD_E_ARG, "trd_match_host: NULL par array");

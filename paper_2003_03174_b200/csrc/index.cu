@@ -28,17 +28,18 @@ constexpr int kTile = kSortThreads * kItems;        // 4096 keys per tile
 // one sector per tracklet instead of three
 __global__ void __launch_bounds__(256) tracklet_key(const float* __restrict__ y, const float* __restrict__ z,
                                                     const float* __restrict__ dydx, const int32_t* __restrict__ chamber,
-                                                    uint32_t* __restrict__ key, float4* __restrict__ packed, int64_t n,
-                                                    IndexGeom g) {
+                                                    const int32_t* __restrict__ interaction, uint32_t* __restrict__ key,
+                                                    float4* __restrict__ packed, int64_t n, IndexGeom g) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     const float yy = y[i], zz = z[i];
     packed[i] = make_float4(yy, zz, dydx[i], __uint_as_float((uint32_t)i));
     const int ch = chamber[i];
     uint32_t k = g.n_bins;                          // unusable: behind every bin
-    if (ch >= 0 && ch < g.n_chambers && isfinite(yy) && isfinite(zz)) {
+    const int ia = (g.n_ia > 1) ? interaction[i] : 0;      // time-frame association: the interaction leads the key
+    if (ch >= 0 && ch < g.n_chambers && isfinite(yy) && isfinite(zz) && ia >= 0 && ia < g.n_ia) {
         const int sector = ch / g.per_sector, layer = ch % g.n_layers;
-        const uint32_t cell = (uint32_t)(sector * g.n_layers + layer);
+        const uint32_t cell = (uint32_t)((ia * g.n_sectors + sector) * g.n_layers + layer);
         k = ((cell * (uint32_t)g.nz + (uint32_t)zrow_of(g, zz)) << g.nb_shift) + (uint32_t)ybin_of(g, yy);
     }
     key[i] = k;
@@ -231,7 +232,7 @@ __global__ void __launch_bounds__(256) gather_store(const uint32_t* __restrict__
                 if (i == n - 1)
                     for (int64_t b = (int64_t)kc + 1; b <= (int64_t)n_bins; ++b) bin_first[b] = (int32_t)n;
             }
-            if (k[u] < n_bins) {
+            if (row_ext && k[u] < n_bins) {
                 row = k[u] >> nb_shift;
                 zlo = zhi = ext_encode(tl[u].y);
             }
@@ -309,11 +310,13 @@ cudaError_t radix_sort_pairs(uint32_t* key0, uint32_t* key1, uint32_t* val0, uin
 }
 
 cudaError_t build_index(trd_handle* h, const float* d_y, const float* d_z, const float* d_dydx,
-                        const int32_t* d_chamber, int64_t n, cudaStream_t stream) {
+                        const int32_t* d_chamber, const int32_t* d_interaction, int n_interactions, int64_t n,
+                        cudaStream_t stream) {
     const trd_config& c = h->cfg;
     IndexGeom& g = h->mp.g;
     // ---- geometry of the bins for this load ----
-    const int n_cells = c.n_sectors * c.n_layers;
+    g.n_ia = (d_interaction && n_interactions > 1) ? n_interactions : 1;
+    const int64_t n_cells = (int64_t)g.n_ia * c.n_sectors * c.n_layers;
     const int half_rows = (int)ceil(c.z_max / c.pad_length) + 1;
     g.nz = 2 * half_rows;
     g.z_off = (float)(half_rows * c.pad_length);
@@ -328,12 +331,14 @@ cudaError_t build_index(trd_handle* h, const float* d_y, const float* d_z, const
         const double per_row = (double)n / ((double)n_cells * g.nz);
         shift = ceil_log2((uint64_t)fmax(per_row / 2.0, 1.0));
     }
-    if (shift < 3) shift = 3;
+    if (shift < 3 && g.n_ia == 1) shift = 3;             // with association a z row of one interaction is nearly empty
+    if (shift < 0) shift = 0;
     if (shift > 10) shift = 10;
-    while (shift > 0 && (uint64_t)n_cells * g.nz * (1ull << shift) >= (1ull << 31)) --shift;
+    while (shift > 0 && (uint64_t)n_cells * g.nz * (1ull << shift) >= (1ull << 28)) --shift;
     g.nb_shift = shift;
     g.y_half = (float)y_half;
     g.inv_w = (float)((double)(1 << shift) / (2.0 * y_half));
+    if ((uint64_t)n_cells * g.nz >= (1ull << 28)) return cudaErrorInvalidValue;     // too many interactions for the key
     g.n_bins = (uint32_t)n_cells * (uint32_t)g.nz * (1u << shift);
     h->ybin_width = 2.0 * y_half / (double)(1 << shift);
     h->key_bits = ceil_log2((uint64_t)g.n_bins + 1);
@@ -342,11 +347,15 @@ cudaError_t build_index(trd_handle* h, const float* d_y, const float* d_z, const
     h->index_loaded = false;
 
     TRD_TRY(reserve(h->bin_first, ((size_t)g.n_bins + 1) * sizeof(int32_t), stream));
-    const size_t n_rows = (size_t)n_cells * g.nz;
-    TRD_TRY(reserve(h->row_ext, n_rows * sizeof(uint2), stream));
-    // empty rows: min = 0xffffffff > max = 0
-    TRD_TRY(cudaMemset2DAsync(h->row_ext.p, sizeof(uint2), 0xff, sizeof(uint32_t), n_rows, stream));
-    TRD_TRY(cudaMemset2DAsync((char*)h->row_ext.p + sizeof(uint32_t), sizeof(uint2), 0x00, sizeof(uint32_t), n_rows, stream));
+    // z extents per row only without association (with it a row holds a couple of tracklets and the table would be large)
+    h->use_row_ext = g.n_ia == 1;
+    if (h->use_row_ext) {
+        const size_t n_rows = (size_t)n_cells * g.nz;
+        TRD_TRY(reserve(h->row_ext, n_rows * sizeof(uint2), stream));
+        // empty rows: min = 0xffffffff > max = 0
+        TRD_TRY(cudaMemset2DAsync(h->row_ext.p, sizeof(uint2), 0xff, sizeof(uint32_t), n_rows, stream));
+        TRD_TRY(cudaMemset2DAsync((char*)h->row_ext.p + sizeof(uint32_t), sizeof(uint2), 0x00, sizeof(uint32_t), n_rows, stream));
+    }
     if (n == 0) {
         TRD_TRY(cudaMemsetAsync(h->bin_first.p, 0, ((size_t)g.n_bins + 1) * sizeof(int32_t), stream));
         h->index_loaded = true;
@@ -363,14 +372,15 @@ cudaError_t build_index(trd_handle* h, const float* d_y, const float* d_z, const
     TRD_TRY(reserve(h->digit_tot, kRadix * sizeof(uint32_t), stream));
 
     const unsigned n_blk = (unsigned)((n + 255) / 256);
-    tracklet_key<<<n_blk, 256, 0, stream>>>(d_y, d_z, d_dydx, d_chamber, (uint32_t*)h->key[0].p, (float4*)h->packed.p, n, g);
+    tracklet_key<<<n_blk, 256, 0, stream>>>(d_y, d_z, d_dydx, d_chamber, d_interaction, (uint32_t*)h->key[0].p,
+                                            (float4*)h->packed.p, n, g);
     h->launches++;
     int side = 0;
     TRD_TRY(radix_sort_pairs((uint32_t*)h->key[0].p, (uint32_t*)h->key[1].p, (uint32_t*)h->val[0].p, (uint32_t*)h->val[1].p,
                              (uint32_t*)h->tile_hist.p, (uint32_t*)h->digit_tot.p, n, h->n_passes, stream, &side, &h->launches));
     h->sorted_side = side;
     gather_store<<<(unsigned)((n + 256 * kGather - 1) / (256 * kGather)), 256, 0, stream>>>((const uint32_t*)h->val[side].p, (const uint32_t*)h->key[side].p,
-                                           (const float4*)h->packed.p, (float4*)h->store.p, (uint2*)h->row_ext.p,
+                                           (const float4*)h->packed.p, (float4*)h->store.p, h->use_row_ext ? (uint2*)h->row_ext.p : nullptr,
                                            (int32_t*)h->bin_first.p, n, g.n_bins, g.nb_shift);
     h->launches += 1;
     TRD_TRY(cudaGetLastError());

@@ -33,7 +33,8 @@ __global__ void __launch_bounds__(kThreads) pack_kernel(const trd_tracks_in in, 
         const int sector = in.sector[i];
         r[20] = x;
         r[21] = __int_as_float(sector);
-        r[22] = 0.0f;
+        const int ia = (g.n_ia > 1) ? in.interaction[i] : 0;
+        r[22] = __int_as_float(ia);
         r[23] = 0.0f;
         // locality key from the straight-line prediction at x_mid
         const float s = fminf(fmaxf(r[2], -0.99f), 0.99f);
@@ -48,7 +49,12 @@ __global__ void __launch_bounds__(kThreads) pack_kernel(const trd_tracks_in in, 
         float fy = floorf((yp + edge_mid) / (2.0f * edge_mid) * (float)(1 << kYBits));
         fy = fminf(fmaxf(fy, 0.0f), (float)((1 << kYBits) - 1));
         const int zr = isfinite(zp) ? zrow_of(g, zp) : 0;
-        key[i] = (((uint32_t)sec * (uint32_t)nz + (uint32_t)zr) << kYBits) + (uint32_t)(isfinite(fy) ? (int)fy : 0);
+        if (g.n_ia > 1) {      // with association the interaction leads, as in the tracklet index
+            const int a = min(max(ia, 0), g.n_ia - 1);
+            key[i] = ((uint32_t)a * (uint32_t)g.n_sectors + (uint32_t)sec) * (uint32_t)nz + (uint32_t)zr;
+        } else {
+            key[i] = (((uint32_t)sec * (uint32_t)nz + (uint32_t)zr) << kYBits) + (uint32_t)(isfinite(fy) ? (int)fy : 0);
+        }
     }
     __syncthreads();
     const int64_t n_here = min((int64_t)kThreads, n - base);
@@ -102,7 +108,7 @@ cudaError_t pack_tracks(trd_handle* h, const trd_tracks_in& in, int64_t n, float
     const unsigned grid = (unsigned)((n + kThreads - 1) / kThreads);
     pack_kernel<<<grid, kThreads, 0, stream>>>(in, n, rec, key, g, x_mid, edge_mid, g.nz);
     h->launches++;
-    uint64_t n_keys = ((uint64_t)c.n_sectors * g.nz) << kYBits;
+    uint64_t n_keys = g.n_ia > 1 ? (uint64_t)g.n_ia * c.n_sectors * g.nz : ((uint64_t)c.n_sectors * g.nz) << kYBits;
     int bits = 0;
     while ((1ull << bits) < n_keys) ++bits;
     *key_bits = bits;

@@ -15,6 +15,7 @@ namespace trd {
 // bin key = (((sector * n_layers + layer) * nz + zrow) << nb_shift) + ybin
 struct IndexGeom {
     int n_sectors, n_layers, per_sector, n_chambers;
+    int n_ia;          // interactions of the loaded time frame (1 = no association)
     int nz;            // z rows per (sector, layer)
     int nb_shift;      // log2(y bins per z row)
     float z_off, inv_pad;
@@ -64,6 +65,7 @@ struct trd_handle {
     int device = 0;
     int sm_count = 0;
     bool index_loaded = false;
+    bool use_row_ext = true;
     int64_t n_tracklets = 0;
     int key_bits = 0, n_passes = 0;
     double ybin_width = 0.0;
@@ -105,7 +107,8 @@ namespace trd {
 
 // returns cudaSuccess or the first error; counts launches into h->launches
 cudaError_t build_index(trd_handle* h, const float* d_y, const float* d_z, const float* d_dydx,
-                        const int32_t* d_chamber, int64_t n, cudaStream_t stream);
+                        const int32_t* d_chamber, const int32_t* d_interaction, int n_interactions, int64_t n,
+                        cudaStream_t stream);
 cudaError_t launch_match(trd_handle* h, const trd_tracks_in& in, const trd_tracks_out& out, int64_t n,
                          cudaStream_t stream);
 

@@ -26,7 +26,11 @@ def run_gpu(B, cfg, data, batch=None, in_place=False):
     n = data["x"].shape[0]
     h = B.trd_create(cfg)
     try:
-        B.trd_load_tracklets(h, dev["tl_y"], dev["tl_z"], dev["tl_dydx"], dev["tl_chamber"])
+        if data.get("n_interactions", 0) > 1:
+            B.trd_load_tracklets_tf(h, dev["tl_y"], dev["tl_z"], dev["tl_dydx"], dev["tl_chamber"], dev["tl_interaction"],
+                                    data["n_interactions"])
+        else:
+            B.trd_load_tracklets(h, dev["tl_y"], dev["tl_z"], dev["tl_dydx"], dev["tl_chamber"])
         if batch is None:
             out = B.alloc_tracks_out(n)
             if in_place:
@@ -39,6 +43,8 @@ def run_gpu(B, cfg, data, batch=None, in_place=False):
             hi = min(n, lo + batch)
             part = dict(par=dev["par"][:, lo:hi].contiguous(), cov=dev["cov"][:, lo:hi].contiguous(),
                         x=dev["x"][lo:hi].contiguous(), sector=dev["sector"][lo:hi].contiguous())
+            if "interaction" in dev:
+                part["interaction"] = dev["interaction"][lo:hi].contiguous()
             parts.append(B.to_numpy(B.trd_match(h, part)))
         return {k: np.concatenate([p[k] for p in parts], axis=-1) for k in parts[0]}
     finally:
@@ -269,3 +275,46 @@ def test_resolution_model_dense(B):
     want = O.match(cfg, d)
     assert want["counters"]["n_cand"] > want["counters"]["n_road"]
     assert_parity(P.compare(run_gpu(B, cfg, d), want), want)
+
+
+@pytest.mark.parametrize("name,n_ia,n_hyp", [("central", 4, 1), ("pileup", 5, 4), ("central8", 7, 8)])
+def test_time_frame_association(B, name, n_ia, n_hyp):
+    """tracklets are matched only to tracks of the same interaction.
+    Pile-up config with its 5 overlapping events as 5 interactions, among others; binned and unbinned batches."""
+    spec = dataclasses.replace(W.CONFIGS[name], n_interactions=n_ia, n_hyp=n_hyp)
+    d = W.generate(spec); cfg = W.matcher_config(spec)
+    want = O.match(cfg, d)
+    got = run_gpu(B, cfg, d)
+    assert_parity(P.compare(got, want), want)
+    assert_parity(P.compare(run_gpu(B, dict(cfg, track_binning=1), d, batch=2111), want), want)
+    att = got["idx"] >= 0                                     # every attached tracklet is of the track's interaction
+    ia_tl = d["tl_interaction"][np.where(att, got["idx"], 0)]
+    assert np.all(ia_tl[att] == np.broadcast_to(d["interaction"], att.shape)[att])
+
+
+def test_time_frame_association_at_scale_and_bad_ids(B):
+    """Config 5's generator at 200k tracks as 100 interactions of 2000 tracks (~2000 tracks per central
+    event), four batches; tracks and tracklets with ids out of range; NULL interaction array -> TRD_E_ARG."""
+    spec = dataclasses.replace(W.scaled(W.CONFIGS["timeframe"], 200_000), n_interactions=100)
+    d = W.generate(spec); cfg = W.matcher_config(spec)
+    d["interaction"][:5] = [-1, 100, 12345, 3, 99]
+    d["tl_interaction"][::97] = 100
+    want = O.match(cfg, d)
+    got = run_gpu(B, cfg, d, batch=50_000)
+    assert_parity(P.compare(got, want), want)
+    assert got["n_matched"][:3].max() == 0
+    import torch
+    h = B.trd_create(cfg)
+    try:
+        dev = B.to_device(d)
+        B.trd_load_tracklets_tf(h, dev["tl_y"], dev["tl_z"], dev["tl_dydx"], dev["tl_chamber"], dev["tl_interaction"], 100)
+        assert B.trd_get_index_info(h)["n_interactions"] == 100
+        no_ia = {k: v for k, v in dev.items() if k != "interaction"}
+        with pytest.raises(B.TrdError) as e:
+            B.trd_match(h, no_ia)
+        assert e.value.code == B.TRD_E_ARG
+        B.trd_load_tracklets(h, dev["tl_y"], dev["tl_z"], dev["tl_dydx"], dev["tl_chamber"])     # back to no association
+        assert B.trd_get_index_info(h)["n_interactions"] == 1
+        B.trd_match(h, no_ia); torch.cuda.synchronize()
+    finally:
+        B.trd_destroy(h)
