@@ -181,13 +181,23 @@ def run_ours(args, spec, cfg):
                    x=dev["x"][lo:hi].contiguous(), sector=dev["sector"][lo:hi].contiguous()) for lo, hi in bounds]
     outs = [B.alloc_tracks_out(hi - lo, device) for lo, hi in bounds]
     tl = (dev["tl_y"], dev["tl_z"], dev["tl_dydx"], dev["tl_chamber"])
+    n_ia = int(data.get("n_interactions", 0))
+    if n_ia > 1:                                 # time-frame association variant (--interactions)
+        for t, (lo, hi) in zip(tracks, bounds):
+            t["interaction"] = dev["interaction"][lo:hi].contiguous()
     h = B.trd_create(cfg)
     stream = torch.cuda.current_stream()
+
+    def load():
+        if n_ia > 1:
+            B.trd_load_tracklets_tf(h, *tl, dev["tl_interaction"], n_ia, stream=stream)
+        else:
+            B.trd_load_tracklets(h, *tl, stream=stream)
 
     def step(ev=None):
         if ev is not None:
             ev.append(torch.cuda.Event(enable_timing=True)); ev[-1].record(stream)
-        B.trd_load_tracklets(h, *tl, stream=stream)
+        load()
         for t, o in zip(tracks, outs):
             if ev is not None:
                 ev.append(torch.cuda.Event(enable_timing=True)); ev[-1].record(stream)
@@ -213,7 +223,7 @@ def run_ours(args, spec, cfg):
     # reading them needs a sync per call, so this runs as a second pass over the same steps
     kern_ms = []
     for _ in range(args.steps):
-        B.trd_load_tracklets(h, *tl, stream=stream)
+        load()
         for t, o in zip(tracks, outs):
             B.trd_match(h, t, o, stream=stream)
             kern_ms.append(B.trd_last_match_kernel_ms(h))
@@ -227,31 +237,33 @@ def run_ours(args, spec, cfg):
     n_evals = int(sum(int(o["n_evals"].sum().item()) for o in outs))
     n_ge2 = int(sum(int((o["n_matched"] >= 2).sum().item()) for o in outs))
 
-    # ---- end to end through the host entry points (pinned host buffers, copies inside the timed region)
-    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy()   # noqa: E731
-    h_tl = [pin(data[k]) for k in ("tl_y", "tl_z", "tl_dydx", "tl_chamber")]
-    h_tracks = [dict(par=pin(data["par"][:, lo:hi]), cov=pin(data["cov"][:, lo:hi]), x=pin(data["x"][lo:hi]),
-                     sector=pin(data["sector"][lo:hi])) for lo, hi in bounds]
-    h_outs = [B.alloc_tracks_out_host(hi - lo, pinned=True) for lo, hi in bounds]
+    e2e_s, e2e_steps = None, 0
+    if n_ia <= 1:
+        # ---- end to end through the host entry points (pinned host buffers, copies inside the timed region)
+        pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy()   # noqa: E731
+        h_tl = [pin(data[k]) for k in ("tl_y", "tl_z", "tl_dydx", "tl_chamber")]
+        h_tracks = [dict(par=pin(data["par"][:, lo:hi]), cov=pin(data["cov"][:, lo:hi]), x=pin(data["x"][lo:hi]),
+                         sector=pin(data["sector"][lo:hi])) for lo, hi in bounds]
+        h_outs = [B.alloc_tracks_out_host(hi - lo, pinned=True) for lo, hi in bounds]
 
-    def step_host():
-        B.trd_load_tracklets_host(h, *h_tl, stream=stream)
-        for t, o in zip(h_tracks, h_outs):
-            B.trd_match_host_async(h, t, o, stream=stream)
-        B.trd_wait_host(h, stream=stream)            # results of all batches are in host memory here
+        def step_host():
+            B.trd_load_tracklets_host(h, *h_tl, stream=stream)
+            for t, o in zip(h_tracks, h_outs):
+                B.trd_match_host_async(h, t, o, stream=stream)
+            B.trd_wait_host(h, stream=stream)            # results of all batches are in host memory here
 
-    for _ in range(2):
-        step_host()
-    torch.cuda.synchronize(); D.barrier()
-    e2e_steps = max(1, min(args.steps, 5))
-    t0 = time.perf_counter()
-    for _ in range(e2e_steps):
-        step_host()
-    torch.cuda.synchronize()
-    e2e_s = D.max_over_ranks(time.perf_counter() - t0, device) / e2e_steps
-    D.barrier()
-    for o, ho in zip(outs, h_outs):               # the two entry points must agree bit for bit
-        assert np.array_equal(o["idx"].cpu().numpy(), ho["idx"]) and np.array_equal(o["chi2"].cpu().numpy(), ho["chi2"])
+        for _ in range(2):
+            step_host()
+        torch.cuda.synchronize(); D.barrier()
+        e2e_steps = max(1, min(args.steps, 5))
+        t0 = time.perf_counter()
+        for _ in range(e2e_steps):
+            step_host()
+        torch.cuda.synchronize()
+        e2e_s = D.max_over_ranks(time.perf_counter() - t0, device) / e2e_steps
+        D.barrier()
+        for o, ho in zip(outs, h_outs):               # the two entry points must agree bit for bit
+            assert np.array_equal(o["idx"].cpu().numpy(), ho["idx"]) and np.array_equal(o["chi2"].cpu().numpy(), ho["chi2"])
     h2d = 16 * n_tl + BYTES_TRACK_IN * n
     d2h = BYTES_TRACK_OUT * n
     info = B.trd_get_index_info(h)
@@ -305,8 +317,10 @@ def run_ours(args, spec, cfg):
                 frac_tracks_ge2_tracklets=n_ge2 / n, index=dict(n_ybins=info["n_ybins"], n_zrows=info["n_zrows"],
                                                                 ybin_width_cm=info["ybin_width"], radix_passes=info["n_passes"]),
                 clocks=clocks, gpu_launches=int(launches),
-                e2e=dict(value=world * n / e2e_s, unit=UNIT, h2d_bytes_per_step=int(h2d), d2h_bytes_per_step=int(d2h),
-                         ms_per_step=1e3 * e2e_s, steps=e2e_steps),
+                e2e=(dict(value=world * n / e2e_s, unit=UNIT, h2d_bytes_per_step=int(h2d), d2h_bytes_per_step=int(d2h),
+                          ms_per_step=1e3 * e2e_s, steps=e2e_steps) if e2e_s else
+                     dict(value=None, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0,
+                          note="the host entry points do not carry interaction ids; device-resident numbers only")),
                 roofline=roof)
     if world == 1 and not args.no_cpu_baseline:
         n_sample = min(ORACLE_SAMPLE_TRACKS, n)
@@ -329,6 +343,8 @@ def main():
     ap.add_argument("--workload", default="timeframe")
     ap.add_argument("--tracks", type=int, default=0, help="scale the workload to this many tracks (debugging)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--interactions", type=int, default=0,
+                    help="> 1: time-frame association with this many interactions (SURVEY.md 8(f) NEXT#2)")
     ap.add_argument("--res-model", type=int, default=0, choices=[0, 1],
                     help="1: inputs and matcher with the sin(phi)-dependent resolutions and pad tilt (SURVEY.md 8(f) NEXT#1)")
     args = ap.parse_args()
@@ -336,9 +352,11 @@ def main():
     spec = W.CONFIGS[args.workload]
     if args.tracks:
         spec = W.scaled(spec, args.tracks)
+    import dataclasses
     if args.res_model:
-        import dataclasses
         spec = dataclasses.replace(spec, res_model=1, name=spec.name + "_res1")
+    if args.interactions > 1:
+        spec = dataclasses.replace(spec, n_interactions=args.interactions, name=spec.name + f"_tf{args.interactions}")
     cfg = W.matcher_config(spec)
     if args.impl == "reference":
         run_reference(args, spec, cfg)
