@@ -133,13 +133,15 @@ def road(cfg: dict, p, c15, layer: int = 0):
     return dict(road_y=out[0], road_z=out[1], tanphi=out[2], Sinv=np.array([[out[3], out[4]], [out[4], out[5]]]))
 
 
-def candidates(cfg: dict, tl: dict, p, c15, sector: int, layer: int, brute: bool = False, cap: int = 4096):
+def candidates(cfg: dict, tl: dict, p, c15, sector: int, layer: int, brute: bool = False, cap: int = 4096,
+               chamber_dx=None):
     """Accepted candidates (caller's tracklet index, chi2 increment) of one state at one layer."""
     y, z, d, ch = (np.ascontiguousarray(tl[k]) for k in ("tl_y", "tl_z", "tl_dydx", "tl_chamber"))
     p = np.array(p, float); c15 = np.array(c15, float)
     oi = np.zeros(cap, np.int32); oc = np.zeros(cap)
     n = lib().orc_candidates(C.byref(make_config(cfg)), _fp(y), _fp(z), _fp(d), _ip(ch), C.c_int64(y.shape[0]),
-                             _dp(p), _dp(c15), int(sector), int(layer), int(brute), _ip(oi), _dp(oc), cap)
+                             _dp(p), _dp(c15), int(sector), int(layer), int(brute), _ip(oi), _dp(oc), cap,
+                             _dp(np.ascontiguousarray(chamber_dx, np.float64)) if chamber_dx is not None else None)
     assert n <= cap
     return oi[:n].copy(), oc[:n].copy()
 
@@ -171,11 +173,17 @@ def match(cfg: dict, data: dict, brute: bool = False, n_threads: int = 0, lo: in
         ia_args = (_ip(tl_ia), _ip(trk_ia), n_ia)
     else:
         ia_args = (None, None, 1)
+    # radial chamber offsets for the two-stage propagation, float64 per chamber, if given
+    dx = data.get("chamber_dx")
+    if dx is not None:
+        dx = np.ascontiguousarray(dx, np.float64)
+        assert dx.shape[0] == cfg["n_sectors"] * cfg["n_stacks"] * cfg["n_layers"]
     rc = lib().orc_match(C.byref(make_config(cfg)), _fp(y), _fp(z), _fp(d), _ip(ch), C.c_int64(y.shape[0]),
                          _fp(par), _fp(cov), _fp(x), _ip(sec), C.c_int64(n), int(brute), int(n_threads),
                          _ip(out["idx"]), _dp(out["par"]), _dp(out["cov"]), _dp(out["x"]), _ip(out["sector"]),
                          _dp(out["chi2"]), _ip(out["n_matched"]), _ip(out["n_evals"]), _dp(out["margin"]),
-                         counters.ctypes.data_as(C.POINTER(C.c_int64)), _dp(seconds), *ia_args)
+                         counters.ctypes.data_as(C.POINTER(C.c_int64)), _dp(seconds), *ia_args,
+                         _dp(dx) if dx is not None else None)
     if rc != 0:
         raise RuntimeError(f"orc_match failed: {rc}")
     out["counters"] = dict(zip(("n_prop", "n_rot", "n_road", "n_cand", "n_upd", "n_scanned"), counters.tolist()))

@@ -72,6 +72,7 @@ struct Tracklet {
     double y, z, dydx;
     int index;         // position in the caller's arrays
     int ia;            // interaction (collision) the tracklet belongs to; 0 without time-frame association [R27]
+    double dx;         // radial offset of the tracklet's chamber from the nominal layer plane [R28]
 };
 
 struct Counters {
@@ -233,10 +234,15 @@ bool propagate_to_layer(const Config& cfg, Hyp& h, double X, double* margin, Cou
 // the coarse one (sigma_z) along it: R = Rot(tau) diag(sy^2, sz^2) Rot(tau)^T, i.e. correlated y-z errors.  The
 // y road is applied to the residual corrected with the extrapolated z, r'_y = r_y - tan(tau) r_z, whose
 // variance is (A S A^T)_yy with A = [[1, -tan(tau)], [0, 1]]; chi2 = r^T S^-1 r is invariant under A.
+// Two-stage propagation [R28-R30]: the hypothesis sits at the nominal ("average") radius of the layer;
+// for the road and chi2 its (y, z) are extrapolated linearly to the radius of each tracklet's chamber,
+// y + dx tan(phi), z + dx tan(lambda) / cos(phi); a kept child is re-propagated exactly to that radius before the
+// Kalman update.
 struct Road {
     double Sinv[2][2];
     double road_y, road_z, tanphi;
     double tan_tilt, veto;
+    double zslope;     // dz/dx of the track = tan(lambda) / cos(phi)
 };
 
 Road make_road(const Config& cfg, const Hyp& h, int layer) {
@@ -267,6 +273,7 @@ Road make_road(const Config& cfg, const Hyp& h, int layer) {
     rd.road_y = cfg.n_sigma_road * std::sqrt(S00 - 2.0 * t * S01 + t * t * S11);     // [R2], of the corrected residual
     rd.road_z = cfg.n_sigma_road * std::sqrt(h.C[1][1]) + 0.5 * cfg.pad_length;      // [R2]
     rd.tanphi = h.p[2] / std::sqrt(1.0 - h.p[2] * h.p[2]);
+    rd.zslope = h.p[3] / std::sqrt(1.0 - h.p[2] * h.p[2]);
     return rd;
 }
 
@@ -298,12 +305,16 @@ double kalman_update(const Config& cfg, Hyp& h, int layer, double ym, double zm)
 // per (sector, layer) and compares the ids tracklet by tracklet -- the two must give identical results.
 struct Store {
     int n_sectors = 0, n_layers = 0, n_ia = 1;
+    double dx_max = 0.0;                       // largest |chamber offset| [R28]
     std::vector<std::vector<Tracklet>> cell;   // [(ia *) sector * n_layers + layer]
     bool sorted = false, by_ia = false;
 };
 
 void build_store(const Config& cfg, const float* y, const float* z, const float* dydx, const int32_t* chamber,
-                 const int32_t* ia, int n_ia, int64_t n, bool sort_by_y, Store& st) {
+                 const int32_t* ia, int n_ia, const double* chamber_dx, int64_t n, bool sort_by_y, Store& st) {
+    st.dx_max = 0.0;
+    if (chamber_dx)
+        for (int c = 0; c < cfg.n_sectors * cfg.n_stacks * cfg.n_layers; ++c) st.dx_max = std::max(st.dx_max, std::fabs(chamber_dx[c]));
     st.n_sectors = cfg.n_sectors;
     st.n_layers = cfg.n_layers;
     st.n_ia = (ia && n_ia > 1) ? n_ia : 1;
@@ -318,7 +329,7 @@ void build_store(const Config& cfg, const float* y, const float* z, const float*
         if (a < 0 || a >= st.n_ia) continue;                                  // no such interaction
         const int sector = ch / per_sector, layer = ch % cfg.n_layers;        // stack id unused [R12]
         const size_t c = ((size_t)(st.by_ia ? a : 0) * cfg.n_sectors + sector) * cfg.n_layers + layer;
-        st.cell[c].push_back({(double)y[i], (double)z[i], (double)dydx[i], (int)i, a});
+        st.cell[c].push_back({(double)y[i], (double)z[i], (double)dydx[i], (int)i, a, chamber_dx ? chamber_dx[ch] : 0.0});
     }
     if (sort_by_y)
         for (auto& v : st.cell)
@@ -330,7 +341,7 @@ void build_store(const Config& cfg, const float* y, const float* z, const float*
 
 struct Cand {
     int index;
-    double y, z, chi2inc;
+    double y, z, chi2inc, dx;
 };
 
 // all tracklets of the hypothesis' sector and layer inside the road, past the inclination
@@ -342,7 +353,7 @@ void find_candidates(const Config& cfg, const Store& st, const Hyp& h, int layer
     const std::vector<Tracklet>& v = st.cell[((size_t)(st.by_ia ? h.ia : 0) * st.n_sectors + h.sector) * st.n_layers + layer];
     size_t lo = 0, hi = v.size();
     if (st.sorted) {
-        const double wide = (rd.road_y + std::fabs(rd.tan_tilt) * rd.road_z) * (1.0 + kLoose);
+        const double wide = (rd.road_y + std::fabs(rd.tan_tilt) * rd.road_z + st.dx_max * std::fabs(rd.tanphi)) * (1.0 + kLoose);
         lo = std::lower_bound(v.begin(), v.end(), h.p[0] - wide,
                               [](const Tracklet& a, double val) { return a.y < val; }) - v.begin();
         hi = std::upper_bound(v.begin(), v.end(), h.p[0] + wide,
@@ -353,7 +364,7 @@ void find_candidates(const Config& cfg, const Store& st, const Hyp& h, int layer
         const Tracklet& tl = v[k];
         if (tl.ia != h.ia) continue;                                         // other interaction [R27]
         if (cnt) cnt->n_scanned++;
-        const double ry = tl.y - h.p[0], rz = tl.z - h.p[1];
+        const double ry = tl.y - (h.p[0] + tl.dx * rd.tanphi), rz = tl.z - (h.p[1] + tl.dx * rd.zslope);   // [R29]
         const double ryc = ry - rd.tan_tilt * rz;                            // y corrected with the extrapolated z
         const double da = std::fabs(tl.dydx - rd.tanphi);
         const bool in_y = std::fabs(ryc) <= rd.road_y, in_z = std::fabs(rz) <= rd.road_z;
@@ -370,14 +381,14 @@ void find_candidates(const Config& cfg, const Store& st, const Hyp& h, int layer
         if (n_evals) (*n_evals)++;                                          // one "candidate evaluation"
         if (cnt) cnt->n_cand++;
         if (c2 >= cfg.chi2_cut) continue;                                   // per-layer cut [R4]
-        out.push_back({tl.index, tl.y, tl.z, c2});
+        out.push_back({tl.index, tl.y, tl.z, c2, tl.dx});
     }
 }
 
 struct Child {
     int parent;        // position of the parent in the current hypothesis list
     int tracklet;      // caller's index, or INT_MAX for the skip-child (sorts after tracklets) [R6]
-    double y, z, score, chi2inc;
+    double y, z, score, chi2inc, dx;
 };
 
 struct TrackResult {
@@ -407,9 +418,9 @@ void match_track(const Config& cfg, const Store& st, const Hyp& seed, TrackResul
                 if (cnt) cnt->n_road++;
                 find_candidates(cfg, st, h, L, rd, cands, &res.n_evals, mg, cnt);
                 for (const Cand& c : cands)
-                    children.push_back({ih, c.index, c.y, c.z, h.score + c.chi2inc, c.chi2inc});
+                    children.push_back({ih, c.index, c.y, c.z, h.score + c.chi2inc, c.chi2inc, c.dx});
             }
-            children.push_back({ih, std::numeric_limits<int>::max(), 0.0, 0.0, h.score + cfg.chi2_penalty, 0.0});
+            children.push_back({ih, std::numeric_limits<int>::max(), 0.0, 0.0, h.score + cfg.chi2_penalty, 0.0, 0.0});
         }
         std::stable_sort(children.begin(), children.end(), [](const Child& a, const Child& b) {
             if (a.score != b.score) return a.score < b.score;
@@ -434,7 +445,19 @@ void match_track(const Config& cfg, const Store& st, const Hyp& seed, TrackResul
             Hyp h = prop[c.parent];
             h.score = c.score;
             if (c.tracklet != std::numeric_limits<int>::max()) {
+                if (c.dx != 0.0) {
+                    // "again propagated ... to the exact radius" before the update [R30].  A track that
+                    // cannot get there keeps its state at the nominal plane, attaches nothing and only skips from now on.
+                    Hyp w = h;
+                    if (!propagate(cfg, w, h.x + c.dx, mg, cnt)) {
+                        h.alive = false;
+                        next.push_back(h);
+                        continue;
+                    }
+                    h = w;
+                }
                 const double chi2inc = kalman_update(cfg, h, L, c.y, c.z);
+                if (c.dx != 0.0) h.score = prop[c.parent].score + chi2inc;   // the exact chi2 replaces the linear estimate
                 if (cnt) cnt->n_upd++;
                 h.chi2 += chi2inc;
                 h.idx[L] = c.tracklet;
@@ -538,9 +561,9 @@ void orc_road(const orc_config* cfg, const double p[5], const double c15[15], do
 // accepted candidates of one state at one layer; returns their number (<= cap written)
 int orc_candidates(const orc_config* cfg, const float* y, const float* z, const float* dydx, const int32_t* chamber,
                    int64_t n, const double p[5], const double c15[15], int sector, int layer, int brute,
-                   int32_t* out_index, double* out_chi2, int cap) {
+                   int32_t* out_index, double* out_chi2, int cap, const double* chamber_dx) {
     Store st;
-    build_store(*cfg, y, z, dydx, chamber, nullptr, 1, n, !brute, st);
+    build_store(*cfg, y, z, dydx, chamber, nullptr, 1, chamber_dx, n, !brute, st);
     Hyp h;
     load_hyp(h, p, c15, cfg->layer_x[layer], sector);
     const Road rd = make_road(*cfg, h, layer);
@@ -564,12 +587,12 @@ int orc_match(const orc_config* cfg, const float* tl_y, const float* tl_z, const
               const int32_t* sector, int64_t n_trk, int brute, int n_threads, int32_t* out_idx, double* out_par,
               double* out_cov, double* out_x, int32_t* out_sector, double* out_chi2, int32_t* out_n_matched,
               int32_t* out_n_evals, double* out_margin, int64_t counters[6], double seconds[2],
-              const int32_t* tl_ia, const int32_t* trk_ia, int32_t n_ia) {
+              const int32_t* tl_ia, const int32_t* trk_ia, int32_t n_ia, const double* chamber_dx) {
     if (cfg->n_layers > kMaxLayers || cfg->n_hyp < 1) return -1;
     if ((tl_ia == nullptr) != (trk_ia == nullptr)) return -2;
     const auto t0 = std::chrono::steady_clock::now();
     Store st;
-    build_store(*cfg, tl_y, tl_z, tl_dydx, tl_chamber, tl_ia, n_ia, n_tl, !brute, st);
+    build_store(*cfg, tl_y, tl_z, tl_dydx, tl_chamber, tl_ia, n_ia, chamber_dx, n_tl, !brute, st);
     const auto t1 = std::chrono::steady_clock::now();
     Counters total;
 #ifdef _OPENMP

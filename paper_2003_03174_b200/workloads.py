@@ -80,6 +80,7 @@ class WorkloadSpec:
     exact_z: bool = False             # tracklet z = true z instead of the pad-row centre
     efficiency: float = EFFICIENCY
     res_model: int = 0                # 1: sigma_y(sin phi), sigma_dydx(sin phi) polynomials and +-2 degree pad tilt
+    chamber_dx_sigma: float = 0.0     # > 0: radial chamber misalignment N(0, sigma) cm, clipped at 3 sigma
     n_interactions: int = 0           # > 1: time-frame association: tracks i*n_ia//n_tracks form one
                                       # collision, their tracklets inherit its id, noise tracklets get a random one
 
@@ -190,6 +191,34 @@ def _truth_at_plane(phi0, kappa, tanl, x_plane):
     return best["sec"], best["y"], best["z"], best["s"], best["ok"]
 
 
+def _truth_in_sector(phi0, kappa, tanl, x_plane, sec):
+    """(y, z, sin(phi), ok) where the particle crosses the plane local-x = x_plane (array) of the GIVEN sector:
+    same circle as _truth_at_plane, no sector search and no edge test (used for radially displaced chambers)."""
+    alpha = (sec + 0.5) * SECTOR_WIDTH
+    ploc = np.mod(phi0 - alpha + np.pi, 2.0 * np.pi) - np.pi
+    s0, c0 = np.sin(ploc), np.cos(ploc)
+    s1 = s0 + kappa * x_plane
+    ok = (np.abs(s1) < 1.0) & (c0 > 0.0)
+    s1c = np.where(ok, s1, 0.0)
+    c1 = np.sqrt(1.0 - s1c * s1c)
+    straight = np.abs(kappa) < 1e-12
+    ksafe = np.where(straight, 1.0, kappa)
+    c0s = np.where(c0 > 0, c0, 1.0)
+    y = np.where(straight, x_plane * s0 / c0s, (c0 - c1) / ksafe)
+    arc = np.where(straight, x_plane / c0s, (np.arcsin(s1c) - ploc) / ksafe)
+    return y, tanl * arc, s1, ok
+
+
+def chamber_offsets(spec: "WorkloadSpec") -> np.ndarray:
+    """Radial offset of every chamber from its nominal layer plane (float32 cm), own seeded stream."""
+    n_ch = N_SECTORS * N_STACKS * N_LAYERS
+    if spec.chamber_dx_sigma <= 0.0:
+        return np.zeros(n_ch, np.float32)
+    rng = np.random.Generator(np.random.PCG64(spec.seed + 1_000_003))
+    sig = spec.chamber_dx_sigma
+    return np.clip(rng.normal(0.0, sig, n_ch), -3.0 * sig, 3.0 * sig).astype(np.float32)
+
+
 def _draw_particles(rng, spec: WorkloadSpec, n: int):
     q = np.where(rng.random(n) < 0.5, -1.0, 1.0)
     if spec.pt_spectrum == "loguniform":
@@ -249,6 +278,7 @@ def generate(spec: WorkloadSpec) -> dict:
     # 3. signal tracklets, layer by layer (draw order per layer: efficiency u, y normal, dy/dx normal)
     sig_y, sig_z, sig_d, sig_ch, sig_lab, sig_lay = [], [], [], [], [], []
     truth_last = np.full((n, 4), np.nan)
+    ch_dx = chamber_offsets(spec)
     for lay, xl in enumerate(LAYER_X):
         secl, yl, zl, sl, okl = _truth_at_plane(phi0, kappa, tanl, xl)
         u = rng.random(n)
@@ -259,6 +289,14 @@ def generate(spec: WorkloadSpec) -> dict:
         if lay == N_LAYERS - 1:
             truth_last[okl] = np.stack([yl, zl, sl, secl.astype(float)], axis=1)[okl]
         idx = np.nonzero(present)[0]
+        chamber_l = secl[idx] * (N_STACKS * N_LAYERS) + stack_of_z(pad_row_centre(zl[idx])) * N_LAYERS + lay
+        if spec.chamber_dx_sigma > 0.0:
+            # the chamber sits at x_l + dx: the tracklet is measured where the particle crosses THAT plane
+            yl, zl, sl = yl.copy(), zl.copy(), sl.copy()
+            yd, zd, sd, okd = _truth_in_sector(phi0[idx], kappa[idx], tanl[idx], xl + ch_dx[chamber_l].astype(np.float64),
+                                               secl[idx])
+            assert okd.all()
+            yl[idx], zl[idx], sl[idx] = yd, zd, sd
         zc = pad_row_centre(zl[idx])
         zz = zl[idx] if spec.exact_z else zc
         tanphi = sl[idx] / np.sqrt(1.0 - sl[idx] ** 2)
@@ -274,7 +312,7 @@ def generate(spec: WorkloadSpec) -> dict:
             yy = yl[idx] + (SIGMA_Y_TRACKLET * ny[idx] if spec.smear_tracklets else 0.0)
             dd = tanphi + (SIGMA_DYDX_TRACKLET * nd[idx] if spec.smear_tracklets else 0.0)
         sig_y.append(yy); sig_z.append(zz); sig_d.append(dd)
-        sig_ch.append(secl[idx] * (N_STACKS * N_LAYERS) + stack_of_z(zc) * N_LAYERS + lay)
+        sig_ch.append(chamber_l)
         sig_lab.append(idx); sig_lay.append(np.full(idx.shape[0], lay))
 
     # 4. noise tracklets (draw order: chamber, y, row pick, dy/dx)
@@ -312,6 +350,8 @@ def generate(spec: WorkloadSpec) -> dict:
     is_sig = tl_lab >= 0
     truth_idx[tl_lab[is_sig], tl_lay[is_sig]] = np.nonzero(is_sig)[0].astype(np.int32)
 
+    if spec.chamber_dx_sigma > 0.0:
+        assoc["chamber_dx"] = ch_dx
     return dict(
         assoc, spec=spec,
         par=np.ascontiguousarray(par, np.float32), cov=np.ascontiguousarray(cov, np.float32),
