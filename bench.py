@@ -187,6 +187,8 @@ def run_ours(args, spec, cfg):
             t["interaction"] = dev["interaction"][lo:hi].contiguous()
     h = B.trd_create(cfg)
     stream = torch.cuda.current_stream()
+    if "chamber_dx" in data:
+        B.trd_set_chamber_dx(h, data["chamber_dx"], stream=stream)
 
     def load():
         if n_ia > 1:
@@ -345,6 +347,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--interactions", type=int, default=0,
                     help="> 1: time-frame association with this many interactions (SURVEY.md 8(f) NEXT#2)")
+    ap.add_argument("--chamber-dx", type=float, default=0.0,
+                    help="> 0: chambers displaced radially by N(0, this) cm, two-stage propagation (SURVEY.md 8(f) NEXT#3)")
     ap.add_argument("--res-model", type=int, default=0, choices=[0, 1],
                     help="1: inputs and matcher with the sin(phi)-dependent resolutions and pad tilt (SURVEY.md 8(f) NEXT#1)")
     args = ap.parse_args()
@@ -357,6 +361,8 @@ def main():
         spec = dataclasses.replace(spec, res_model=1, name=spec.name + "_res1")
     if args.interactions > 1:
         spec = dataclasses.replace(spec, n_interactions=args.interactions, name=spec.name + f"_tf{args.interactions}")
+    if args.chamber_dx > 0.0:
+        spec = dataclasses.replace(spec, chamber_dx_sigma=args.chamber_dx, name=spec.name + "_dx")
     cfg = W.matcher_config(spec)
     if args.impl == "reference":
         run_reference(args, spec, cfg)

@@ -157,6 +157,14 @@ int trd_load_tracklets_tf(trd_handle* h, const float* d_y, const float* d_z, con
                           const int32_t* d_chamber, const int32_t* d_interaction, int32_t n_interactions, int64_t n,
                           void* stream);
 
+/* Two-stage propagation: radial offset [cm] of every chamber from its nominal layer plane, HOST
+ * array of n_chambers = n_sectors * n_stacks * n_layers floats (copied; NULL or 0 chambers = all nominal).  A
+ * hypothesis is extrapolated to the nominal plane ("average radius"); its (y, z) are extrapolated linearly to
+ * x_layer + dx of each candidate's chamber for the road and the chi2; a selected child is re-propagated exactly to
+ * that radius before the Kalman update, so the output x is x_layer + dx of the last attached chamber.  Takes effect
+ * with the NEXT trd_load_tracklets (the loaded index is dropped). */
+int trd_set_chamber_dx(trd_handle* h, const float* dx, int32_t n_chambers, void* stream);
+
 /* The tracking step for one batch (n_tracks >= 0) against the loaded index. */
 int trd_match(trd_handle* h, const trd_tracks_in* in, const trd_tracks_out* out, int64_t n_tracks,
               void* stream);

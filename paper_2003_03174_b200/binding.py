@@ -20,7 +20,7 @@ TRD_MAX_HYP = 8
 TRD_OK, TRD_E_ARG, TRD_E_CUDA, TRD_E_NOMEM, TRD_E_STATE = 0, -1, -2, -3, -4
 _STATUS = {0: "TRD_OK", -1: "TRD_E_ARG", -2: "TRD_E_CUDA", -3: "TRD_E_NOMEM", -4: "TRD_E_STATE"}
 
-EXPORTS = ("trd_version", "trd_create", "trd_destroy", "trd_load_tracklets", "trd_load_tracklets_tf", "trd_match",
+EXPORTS = ("trd_version", "trd_create", "trd_destroy", "trd_load_tracklets", "trd_load_tracklets_tf", "trd_set_chamber_dx", "trd_match",
            "trd_load_tracklets_host", "trd_match_host", "trd_match_host_async", "trd_wait_host", "trd_get_index_info", "trd_copy_index",
            "trd_last_error", "trd_device_bytes", "trd_kernel_launches", "trd_last_match_kernel_ms")
 
@@ -87,6 +87,7 @@ def lib():
         l.trd_load_tracklets_host.argtypes = l.trd_load_tracklets.argtypes
         l.trd_load_tracklets_tf.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32,
                                             C.c_int64, C.c_void_p]
+        l.trd_set_chamber_dx.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]
         l.trd_match.argtypes = [C.c_void_p, C.POINTER(TrdTracksIn), C.POINTER(TrdTracksOut), C.c_int64, C.c_void_p]
         l.trd_match_host.argtypes = l.trd_match.argtypes
         l.trd_match_host_async.argtypes = l.trd_match.argtypes
@@ -176,6 +177,14 @@ def trd_load_tracklets_tf(h, d_y, d_z, d_dydx, d_chamber, d_interaction, n_inter
     _check(h, lib().trd_load_tracklets_tf(h, _dev_ptr(d_y, "f32", n), _dev_ptr(d_z, "f32", n), _dev_ptr(d_dydx, "f32", n),
                                           _dev_ptr(d_chamber, "i32", n), _dev_ptr(d_interaction, "i32", n),
                                           int(n_interactions), n, _stream(stream)))
+
+
+def trd_set_chamber_dx(h, dx: Optional[np.ndarray], stream=None) -> None:
+    """Radial chamber offsets (float32 numpy array, one per chamber) for the two-stage propagation; None clears."""
+    if dx is None:
+        _check(h, lib().trd_set_chamber_dx(h, None, 0, _stream(stream)))
+    else:
+        _check(h, lib().trd_set_chamber_dx(h, _host_ptr(dx, np.float32), int(dx.size), _stream(stream)))
 
 
 def alloc_tracks_out(n: int, device="cuda", with_evals: bool = True) -> Dict[str, "object"]:

@@ -139,6 +139,8 @@ void trd_destroy(trd_handle* h) {
     release(h->digit_tot);
     release(h->bin_first);
     release(h->row_ext);
+    release(h->chamber_dx);
+    release(h->store_dx);
     trd::host_pipeline_destroy(h);
     release(h->trk_rec);
     release(h->trk_out);
@@ -173,6 +175,29 @@ int trd_load_tracklets_tf(trd_handle* h, const float* d_y, const float* d_z, con
     const cudaError_t e = trd::build_index(h, d_y, d_z, d_dydx, d_chamber, d_interaction, n_interactions, n, (cudaStream_t)stream);
     if (e == cudaErrorInvalidValue) return fail(h, TRD_E_ARG, "trd_load_tracklets_tf: interactions x rows exceed the key range");
     if (e != cudaSuccess) return fail_cuda(h, e, "trd_load_tracklets_tf");
+    return TRD_OK;
+}
+
+int trd_set_chamber_dx(trd_handle* h, const float* dx, int32_t n_chambers, void* stream) {
+    if (!h) return TRD_E_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (!dx || n_chambers == 0) {                        // back to the nominal planes
+        h->mp.dx_max = 0.0f;
+        h->index_loaded = false;
+        return TRD_OK;
+    }
+    if (n_chambers != h->mp.g.n_chambers) return fail(h, TRD_E_ARG, "trd_set_chamber_dx: n_chambers does not match the geometry");
+    float mx = 0.0f;
+    for (int c = 0; c < n_chambers; ++c) {
+        if (!isfinite(dx[c])) return fail(h, TRD_E_ARG, "trd_set_chamber_dx: offset not finite");
+        mx = fmaxf(mx, fabsf(dx[c]));
+    }
+    cudaError_t e = trd::reserve(h->chamber_dx, (size_t)n_chambers * sizeof(float), st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(h->chamber_dx.p, dx, (size_t)n_chambers * sizeof(float), cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);  // dx may be pageable and freed by the caller
+    if (e != cudaSuccess) return fail_cuda(h, e, "trd_set_chamber_dx");
+    h->mp.dx_max = mx;
+    h->index_loaded = false;                             // the next trd_load_tracklets picks the offsets up
     return TRD_OK;
 }
 
@@ -231,7 +256,7 @@ const char* trd_last_error(const trd_handle* h) { return h ? h->err.c_str() : "N
 
 int64_t trd_device_bytes(const trd_handle* h) {
     if (!h) return 0;
-    size_t t = h->store.bytes + h->packed.bytes + h->tile_hist.bytes + h->digit_tot.bytes + h->bin_first.bytes + h->row_ext.bytes + h->stage_tl.bytes + h->trk_rec.bytes + h->trk_out.bytes + h->trk_hist.bytes +
+    size_t t = h->store.bytes + h->packed.bytes + h->tile_hist.bytes + h->digit_tot.bytes + h->bin_first.bytes + h->row_ext.bytes + h->chamber_dx.bytes + h->store_dx.bytes + h->stage_tl.bytes + h->trk_rec.bytes + h->trk_out.bytes + h->trk_hist.bytes +
                h->trk_tot.bytes;
     for (int s = 0; s < 2; ++s) t += h->key[s].bytes + h->val[s].bytes + h->trk_key[s].bytes + h->trk_val[s].bytes;
     return (int64_t)t;

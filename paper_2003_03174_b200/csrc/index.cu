@@ -24,7 +24,7 @@ constexpr int kSortWarps = kSortThreads / 32;
 constexpr int kItems = 16;                          // keys per thread and tile
 constexpr int kTile = kSortThreads * kItems;        // 4096 keys per tile
 
-// also packs (y, z, dy/dx, position) into one 16-byte record so that the gather after the sort reads
+// also packs (y, z, dy/dx, chamber) into one 16-byte record so that the gather after the sort reads
 // one sector per tracklet instead of three
 __global__ void __launch_bounds__(256) tracklet_key(const float* __restrict__ y, const float* __restrict__ z,
                                                     const float* __restrict__ dydx, const int32_t* __restrict__ chamber,
@@ -33,7 +33,7 @@ __global__ void __launch_bounds__(256) tracklet_key(const float* __restrict__ y,
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     const float yy = y[i], zz = z[i];
-    packed[i] = make_float4(yy, zz, dydx[i], __uint_as_float((uint32_t)i));
+    packed[i] = make_float4(yy, zz, dydx[i], __int_as_float(chamber[i]));
     const int ch = chamber[i];
     uint32_t k = g.n_bins;                          // unusable: behind every bin
     const int ia = (g.n_ia > 1) ? interaction[i] : 0;      // time-frame association: the interaction leads the key
@@ -204,16 +204,18 @@ constexpr int kGather = 4;
 
 __global__ void __launch_bounds__(256) gather_store(const uint32_t* __restrict__ pos, const uint32_t* __restrict__ key,
                                                     const float4* __restrict__ packed, float4* __restrict__ store,
-                                                    uint2* __restrict__ row_ext, int32_t* __restrict__ bin_first, int64_t n,
-                                                    uint32_t n_bins, int nb_shift) {
+                                                    uint2* __restrict__ row_ext, int32_t* __restrict__ bin_first,
+                                                    const float* __restrict__ chamber_dx, float* __restrict__ store_dx,
+                                                    int n_chambers, int64_t n, uint32_t n_bins, int nb_shift) {
     const int64_t base = (int64_t)blockIdx.x * (256 * kGather) + threadIdx.x;
     float4 tl[kGather];
-    uint32_t k[kGather], kprev[kGather];
+    uint32_t k[kGather], kprev[kGather], p[kGather];
 #pragma unroll
     for (int u = 0; u < kGather; ++u) {
         const int64_t i = base + u * 256;
         if (i < n) {
-            tl[u] = __ldg(packed + pos[i]);
+            p[u] = pos[i];
+            tl[u] = __ldg(packed + p[u]);
             k[u] = key[i];
             kprev[u] = (i == 0) ? 0u : key[i - 1];
         }
@@ -224,7 +226,9 @@ __global__ void __launch_bounds__(256) gather_store(const uint32_t* __restrict__
         const bool ok = i < n;
         uint32_t row = 0xffffffffu, zlo = 0xffffffffu, zhi = 0u;
         if (ok) {
-            store[i] = tl[u];
+            const int ch = __float_as_int(tl[u].w);
+            store[i] = make_float4(tl[u].x, tl[u].y, tl[u].z, __uint_as_float(p[u]));      // (y, z, dy/dx, position)
+            if (store_dx) store_dx[i] = (ch >= 0 && ch < n_chambers) ? __ldg(chamber_dx + ch) : 0.0f;
             {   // a3: bin_first[b] = first sorted position whose key is >= b, for b = 0..n_bins (boundary detection)
                 const uint32_t kc = min(k[u], n_bins);
                 const int64_t lo = (i == 0) ? 0 : (int64_t)min(kprev[u], n_bins) + 1;
@@ -364,6 +368,8 @@ cudaError_t build_index(trd_handle* h, const float* d_y, const float* d_z, const
     const int n_tiles = (int)((n + kTile - 1) / kTile);
     TRD_TRY(reserve(h->store, (size_t)n * sizeof(float4), stream));
     TRD_TRY(reserve(h->packed, (size_t)n * sizeof(float4), stream));
+    const bool has_dx = h->mp.dx_max > 0.0f;
+    if (has_dx) TRD_TRY(reserve(h->store_dx, (size_t)n * sizeof(float), stream));
     for (int s = 0; s < 2; ++s) {
         TRD_TRY(reserve(h->key[s], (size_t)n * sizeof(uint32_t), stream));
         TRD_TRY(reserve(h->val[s], (size_t)n * sizeof(uint32_t), stream));
@@ -381,7 +387,8 @@ cudaError_t build_index(trd_handle* h, const float* d_y, const float* d_z, const
     h->sorted_side = side;
     gather_store<<<(unsigned)((n + 256 * kGather - 1) / (256 * kGather)), 256, 0, stream>>>((const uint32_t*)h->val[side].p, (const uint32_t*)h->key[side].p,
                                            (const float4*)h->packed.p, (float4*)h->store.p, h->use_row_ext ? (uint2*)h->row_ext.p : nullptr,
-                                           (int32_t*)h->bin_first.p, n, g.n_bins, g.nb_shift);
+                                           (int32_t*)h->bin_first.p, has_dx ? (const float*)h->chamber_dx.p : nullptr,
+                                           has_dx ? (float*)h->store_dx.p : nullptr, g.n_chambers, n, g.n_bins, g.nb_shift);
     h->launches += 1;
     TRD_TRY(cudaGetLastError());
     h->index_loaded = true;

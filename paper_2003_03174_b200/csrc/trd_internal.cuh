@@ -50,6 +50,8 @@ struct MatchParams {
     // measurement model (res_model = 1: PAPER.md:62, 66)
     int res_model;
     float n_sigma_angle, sy_c0, sy_c2, sd_c0, sd_c2, sin_lorentz, tan_tilt;
+    // two-stage propagation: largest |radial chamber offset|, 0 = all chambers on their nominal plane
+    float dx_max;
 };
 
 struct Buffer {
@@ -82,6 +84,8 @@ struct trd_handle {
     trd::Buffer digit_tot;  // [256]
     trd::Buffer bin_first;  // [n_bins + 1]
     trd::Buffer row_ext;    // uint2 per (cell, z row): encoded min and max z of the row
+    trd::Buffer chamber_dx; // float per chamber: radial offset from the nominal layer plane (trd_set_chamber_dx)
+    trd::Buffer store_dx;   // float per sorted tracklet: the offset of its chamber (only when offsets are set)
     int sorted_side = 0;    // which of key[]/val[] holds the sorted result
     // staging for the *_host entry points
     trd::Buffer stage_tl;   // tracklets

@@ -26,6 +26,8 @@ def run_gpu(B, cfg, data, batch=None, in_place=False):
     n = data["x"].shape[0]
     h = B.trd_create(cfg)
     try:
+        if "chamber_dx" in data:
+            B.trd_set_chamber_dx(h, np.ascontiguousarray(data["chamber_dx"], np.float32))
         if data.get("n_interactions", 0) > 1:
             B.trd_load_tracklets_tf(h, dev["tl_y"], dev["tl_z"], dev["tl_dydx"], dev["tl_chamber"], dev["tl_interaction"],
                                     data["n_interactions"])
@@ -318,3 +320,34 @@ def test_time_frame_association_at_scale_and_bad_ids(B):
         B.trd_match(h, no_ia); torch.cuda.synchronize()
     finally:
         B.trd_destroy(h)
+
+
+@pytest.mark.parametrize("name,n_hyp,extra", [("central", 1, {}), ("pileup", 4, {}), ("central8", 8, dict(res_model=1, n_interactions=3))])
+def test_two_stage_propagation_with_displaced_chambers(B, name, n_hyp, extra):
+    """chambers displaced radially by N(0, 0.3 cm); linear extrapolation for
+    road and chi2, exact re-propagation before the update; also combined with the resolution model and association."""
+    spec = dataclasses.replace(W.CONFIGS[name], chamber_dx_sigma=0.3, n_hyp=n_hyp, **extra)
+    d = W.generate(spec); cfg = W.matcher_config(spec)
+    want = O.match(cfg, d)
+    got = run_gpu(B, cfg, d)
+    assert_parity(P.compare(got, want, x_atol=1e-4), want)
+    assert_parity(P.compare(run_gpu(B, dict(cfg, track_binning=1), d, batch=1999), want, x_atol=1e-4), want)
+    assert np.abs(got["x"] - 364.0).max() > 0.3                       # states live at the displaced radii
+    # the offsets matter, and clearing them gives the plain matcher again
+    plain_want = O.match(cfg, {k: v for k, v in d.items() if k != "chamber_dx"})
+    assert plain_want["n_matched"].sum() < 0.98 * want["n_matched"].sum()
+    h = B.trd_create(cfg)
+    try:
+        B.trd_set_chamber_dx(h, d["chamber_dx"])
+        B.trd_set_chamber_dx(h, None)
+        dev = B.to_device(d)
+        with pytest.raises(B.TrdError) as e:                          # the index was dropped
+            B.trd_match(h, dev)
+        assert e.value.code == B.TRD_E_STATE
+        with pytest.raises(B.TrdError) as e:
+            B.trd_set_chamber_dx(h, np.zeros(17, np.float32))
+        assert e.value.code == B.TRD_E_ARG
+    finally:
+        B.trd_destroy(h)
+    no_dx = {k: v for k, v in d.items() if k != "chamber_dx"}
+    assert_parity(P.compare(run_gpu(B, cfg, no_dx), plain_want), plain_want)
