@@ -24,9 +24,10 @@ EPS_MARGIN = 1e-4
 
 
 def compare(got: Dict[str, np.ndarray], want: Dict[str, np.ndarray], eps_margin: float = EPS_MARGIN,
-            chi2_atol: float = 0.0, cov_rtol: float = 2e-3, x_atol: float = 0.0) -> dict:
+            chi2_atol: float = 0.0, cov_rtol: float = 2e-3, x_atol: float = 0.0, par_atol: float = PAR_ATOL) -> dict:
     """x_atol: tolerance on the output x; 0 (exact) unless chambers are radially displaced, where x = x_layer + dx
-    is a float32 sum on one side and a double sum on the other."""
+    is a float32 sum on one side and a double sum on the other.  par_atol: the absolute floor of the parameter
+    tolerance; the north_star's 1e-5 on the five configs, wider only for stress inputs outside them."""
     n = want["x"].shape[0]
     same = np.all(got["idx"][:, :n] == want["idx"], axis=0)
     fragile = want["margin"] < eps_margin
@@ -38,7 +39,7 @@ def compare(got: Dict[str, np.ndarray], want: Dict[str, np.ndarray], eps_margin:
     s = same
     gp = got["par"][:, :n].astype(np.float64)
     dp = np.abs(gp - want["par"])
-    par_ok = (dp <= PAR_RTOL * np.abs(want["par"])) | (dp <= PAR_ATOL)
+    par_ok = (dp <= PAR_RTOL * np.abs(want["par"])) | (dp <= par_atol)
     bad_par = s & ~np.all(par_ok, axis=0)
     rep["n_par_bad"] = int(bad_par.sum())
     rep["par_bad_tracks"] = np.nonzero(bad_par)[0][:20].tolist()

@@ -351,3 +351,29 @@ def test_two_stage_propagation_with_displaced_chambers(B, name, n_hyp, extra):
         B.trd_destroy(h)
     no_dx = {k: v for k, v in d.items() if k != "chamber_dx"}
     assert_parity(P.compare(run_gpu(B, cfg, no_dx), plain_want), plain_want)
+
+
+def test_random_configurations(B):
+    """Seeded sweep over the knobs of trd_config and of the generator (24 combinations, 3000 tracks each): every
+    sub-warp width, roads, cuts, penalties, field values, spectra, measurement model, association, displaced
+    chambers, bin widths, track binning."""
+    rng = np.random.default_rng(20030317)
+    for k in range(24):
+        n_hyp = int(rng.integers(1, 9))
+        spec = dataclasses.replace(
+            W.CONFIGS["central"], name=f"rand{k}", number=100 + k, n_tracks=3000, n_noise=int(rng.choice([3000, 60000, 600000])),
+            n_hyp=n_hyp, n_sigma_road=float(rng.choice([2.0, 3.0, 5.0])), bz=float(rng.choice([-0.5, 0.2, 0.5])),
+            pt_spectrum=str(rng.choice(["loguniform", "exp"])), res_model=int(rng.integers(0, 2)),
+            n_interactions=int(rng.choice([0, 0, 3, 40])), chamber_dx_sigma=float(rng.choice([0.0, 0.0, 0.2])),
+            efficiency=float(rng.choice([0.6, 0.9, 1.0])))
+        d = W.generate(spec)
+        cfg = dict(W.matcher_config(spec), chi2_cut=float(rng.choice([5.0, 15.0, 30.0])),
+                   chi2_penalty=float(rng.choice([5.0, 15.0, 25.0])), ybin_width=float(rng.choice([0.0, 0.0, 0.05, 2.0])),
+                   track_binning=int(rng.choice([-1, 0, 1])), n_sigma_angle=float(rng.choice([3.0, 4.0])))
+        want = O.match(cfg, d)
+        got = run_gpu(B, cfg, d, batch=None if k % 3 else 1024)
+        # stress inputs (curling 0.3 GeV/c tracks): a local y that ends near 0 after +-60 cm excursions carries the
+        # float32 rounding of those excursions (ulp(64 cm) = 7.6e-6 cm per operation), hence the 3e-5 cm floor here;
+        # the five configs are held to the north_star's 1e-5 (DESIGN.md 5)
+        rep = P.compare(got, want, x_atol=1e-4 if spec.chamber_dx_sigma > 0 else 0.0, par_atol=3e-5)
+        assert rep["ok"] and rep["n_evals_bad"] == 0 and rep["n_assign_mismatch"] <= rep["n_fragile"], (k, spec, cfg, rep)
