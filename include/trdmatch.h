@@ -7,7 +7,7 @@
  * inclination is more than n_sigma_angle sigma off the track inclination are excluded
  * (PAPER.md:60), the best n_hyp hypotheses per layer are kept (Fig. 2) and updated
  * with a Kalman filter.  The paper prints no equation for any of this; the
- * readings taken are listed in DESIGN.md ("Readings", R1..R23).
+ * readings taken are listed in DESIGN.md ("Readings", R1..R30).
  *
  * Conventions: cm, Tesla, GeV/c.  Sector frame s is rotated by (s + 1/2) * 2pi/n_sectors about
  * the beam axis; the state at local x is (y, z, sin(phi), tan(lambda), q/pT); curvature
