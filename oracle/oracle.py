@@ -19,6 +19,7 @@ _LIB = os.path.join(_HERE, "build", "libtrd_oracle.so")
 _lib = None
 
 N_LAYERS_MAX = 6
+REFIT_VAR = (1.0, 25.0, 2.5e-3, 2.5e-3, 0.25)     # default reset variances of the TRD-only refit [R31]
 
 
 class OrcConfig(C.Structure):
@@ -31,6 +32,7 @@ class OrcConfig(C.Structure):
         ("chi2_cut", C.c_double), ("chi2_penalty", C.c_double), ("max_snp", C.c_double),
         ("sy_c0", C.c_double), ("sy_c2", C.c_double), ("sd_c0", C.c_double), ("sd_c2", C.c_double),
         ("sin_lorentz", C.c_double), ("tan_tilt", C.c_double), ("res_model", C.c_int32), ("pad_", C.c_int32),
+        ("x_ref", C.c_double), ("refit_var", C.c_double * 5),
     ]
 
 
@@ -67,6 +69,9 @@ def make_config(cfg: dict) -> OrcConfig:
     for k in ("sy_c0", "sy_c2", "sd_c0", "sd_c2", "sin_lorentz", "tan_tilt"):
         setattr(c, k, float(cfg.get(k, 0.0)))
     c.res_model = int(cfg.get("res_model", 0))
+    c.x_ref = float(cfg.get("x_ref", 247.0))
+    for i, v in enumerate(cfg.get("refit_var", REFIT_VAR)):
+        c.refit_var[i] = float(v)
     return c
 
 
@@ -188,6 +193,28 @@ def match(cfg: dict, data: dict, brute: bool = False, n_threads: int = 0, lo: in
         raise RuntimeError(f"orc_match failed: {rc}")
     out["counters"] = dict(zip(("n_prop", "n_rot", "n_road", "n_cand", "n_upd", "n_scanned"), counters.tolist()))
     out["seconds"] = dict(index=float(seconds[0]), match=float(seconds[1]))
+    return out
+
+
+def refit(cfg: dict, data: dict, matched: dict, min_tracklets: int = 2) -> dict:
+    """TRD-only inward refit of the chains in `matched` (the dict returned by match, or the CUDA path's output widened
+    to float64) to the plane x_ref.  Returns par, cov, x, sector, chi2, n_used."""
+    y, z, ch = (np.ascontiguousarray(data[k]) for k in ("tl_y", "tl_z", "tl_chamber"))
+    n = matched["x"].shape[0]
+    idx = np.ascontiguousarray(matched["idx"], np.int32)
+    par = np.ascontiguousarray(matched["par"], np.float64); cov = np.ascontiguousarray(matched["cov"], np.float64)
+    x = np.ascontiguousarray(matched["x"], np.float64); sec = np.ascontiguousarray(matched["sector"], np.int32)
+    dx = data.get("chamber_dx")
+    if dx is not None:
+        dx = np.ascontiguousarray(dx, np.float64)
+    out = dict(par=np.zeros((5, n)), cov=np.zeros((15, n)), x=np.zeros(n), sector=np.zeros(n, np.int32),
+               chi2=np.zeros(n), n_used=np.zeros(n, np.int32))
+    rc = lib().orc_refit(C.byref(make_config(cfg)), _fp(y), _fp(z), _ip(ch), C.c_int64(y.shape[0]),
+                         _dp(dx) if dx is not None else None, _ip(idx), _dp(par), _dp(cov), _dp(x), _ip(sec), C.c_int64(n),
+                         int(min_tracklets), _dp(out["par"]), _dp(out["cov"]), _dp(out["x"]), _ip(out["sector"]),
+                         _dp(out["chi2"]), _ip(out["n_used"]))
+    if rc != 0:
+        raise RuntimeError(f"orc_refit failed: {rc}")
     return out
 
 

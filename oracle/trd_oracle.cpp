@@ -53,6 +53,8 @@ struct Config {
     // measurement model of PAPER.md:62 (Fig. 3) and PAPER.md:66, readings [R24-R26]; res_model = 0: constants
     double sy_c0, sy_c2, sd_c0, sd_c2, sin_lorentz, tan_tilt;
     int32_t res_model, pad_;
+    // TRD-only refit (PAPER.md:33 step 3) [R31]: reference plane and the variances the covariance is reset to
+    double x_ref, refit_var[5];
 };
 
 struct Hyp {
@@ -638,6 +640,62 @@ int orc_match(const orc_config* cfg, const float* tl_y, const float* tl_z, const
     if (seconds) {
         seconds[0] = std::chrono::duration<double>(t1 - t0).count();
         seconds[1] = std::chrono::duration<double>(t2 - t1).count();
+    }
+    return 0;
+}
+
+// TRD-only refit of the matched chains (calibration step 3: "refits ... ignoring the TPC clusters";
+// PAPER.md:9) [R31].  For every track with at least min_tracklets attached tracklets (two): start from the
+// matched final state, reset the covariance to diag(refit_var) so that nothing of the seed's (TPC) information
+// enters, run the Kalman filter INWARD over the attached tracklets only (propagation to each tracklet's plane with
+// the sector rule of the matcher, update with the measurement model of the matcher), then propagate to x_ref.
+// in_*: the matcher's outputs (double, SoA).  out_n_used < min_tracklets marks a track that was not refitted
+// (state copied through).  A tracklet whose chamber is not in the state's sector frame is skipped.
+int orc_refit(const orc_config* cfg, const float* tl_y, const float* tl_z, const int32_t* tl_chamber, int64_t n_tl,
+              const double* chamber_dx, const int32_t* in_idx, const double* in_par, const double* in_cov, const double* in_x,
+              const int32_t* in_sector, int64_t n_trk, int min_tracklets, double* out_par, double* out_cov, double* out_x,
+              int32_t* out_sector, double* out_chi2, int32_t* out_n_used) {
+    const int per_sector = cfg->n_stacks * cfg->n_layers;
+    for (int64_t i = 0; i < n_trk; ++i) {
+        double p[5], c15[15];
+        for (int k = 0; k < 5; ++k) p[k] = in_par[k * n_trk + i];
+        for (int k = 0; k < 15; ++k) c15[k] = in_cov[k * n_trk + i];
+        Hyp h;
+        load_hyp(h, p, c15, in_x[i], in_sector[i]);
+        int n_att = 0;
+        for (int l = 0; l < cfg->n_layers; ++l) n_att += in_idx[l * n_trk + i] >= 0;
+        int n_used = 0;
+        double chi2 = 0.0;
+        bool ok = n_att >= min_tracklets && std::fabs(p[2]) < cfg->max_snp;
+        if (ok) {
+            for (int a = 0; a < 5; ++a)
+                for (int b = 0; b < 5; ++b) h.C[a][b] = (a == b) ? cfg->refit_var[a] : 0.0;
+            for (int l = cfg->n_layers - 1; l >= 0 && ok; --l) {
+                const int k = in_idx[l * n_trk + i];
+                if (k < 0 || k >= n_tl) continue;
+                const int ch = tl_chamber[k];
+                const double X = cfg->layer_x[l] + (chamber_dx ? chamber_dx[ch] : 0.0);
+                if (h.x != X) ok = propagate_to_layer(*cfg, h, X, nullptr, nullptr);
+                if (!ok) break;
+                if (ch / per_sector != h.sector) continue;           // attached in another frame: not used
+                chi2 += kalman_update(*cfg, h, l, (double)tl_y[k], (double)tl_z[k]);
+                ++n_used;
+                if (std::fabs(h.p[2]) >= cfg->max_snp) ok = false;
+            }
+            if (ok) ok = propagate_to_layer(*cfg, h, cfg->x_ref, nullptr, nullptr);
+        }
+        if (!ok) {                                                   // not refitted: the matcher's state goes through
+            load_hyp(h, p, c15, in_x[i], in_sector[i]);
+            n_used = 0;
+            chi2 = 0.0;
+        }
+        for (int k = 0; k < 5; ++k) out_par[k * n_trk + i] = h.p[k];
+        store_cov(h, c15);
+        for (int k = 0; k < 15; ++k) out_cov[k * n_trk + i] = c15[k];
+        out_x[i] = h.x;
+        out_sector[i] = h.sector;
+        out_chi2[i] = chi2;
+        out_n_used[i] = n_used;
     }
     return 0;
 }
