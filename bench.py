@@ -230,6 +230,16 @@ def run_ours(args, spec, cfg):
             B.trd_match(h, t, o, stream=stream)
             kern_ms.append(B.trd_last_match_kernel_ms(h))
     torch.cuda.synchronize(); D.barrier()
+    # TRD-only refit of the matched chains: reported beside the step, not part of it
+    r_outs = [B.trd_refit(h, o, stream=stream) for o in outs]
+    torch.cuda.synchronize()
+    r0 = torch.cuda.Event(enable_timing=True); r1 = torch.cuda.Event(enable_timing=True)
+    r0.record(stream)
+    for o, ro in zip(outs, r_outs):
+        B.trd_refit(h, o, ro, stream=stream)
+    r1.record(stream); torch.cuda.synchronize()
+    refit_ms = r0.elapsed_time(r1)
+    n_refitted = int(sum(int((ro["n_used"] >= 2).sum().item()) for ro in r_outs))
     total_ms = D.max_over_ranks(t_start.elapsed_time(t_end), device)
     ms_per_step = total_ms / args.steps
     value = world * n / (ms_per_step * 1e-3)
@@ -318,6 +328,8 @@ def run_ours(args, spec, cfg):
                 cand_evals_per_s=world * n_evals / (ms_per_step * 1e-3), n_cand_evals=n_evals,
                 frac_tracks_ge2_tracklets=n_ge2 / n, index=dict(n_ybins=info["n_ybins"], n_zrows=info["n_zrows"],
                                                                 ybin_width_cm=info["ybin_width"], radix_passes=info["n_passes"]),
+                refit=dict(ms_per_time_frame=refit_ms, tracks_per_s=n / (refit_ms * 1e-3), frac_refitted=n_refitted / n,
+                           note="trd_refit over the matched chains of the step, device-resident, timed separately"),
                 clocks=clocks, gpu_launches=int(launches),
                 e2e=(dict(value=world * n / e2e_s, unit=UNIT, h2d_bytes_per_step=int(h2d), d2h_bytes_per_step=int(d2h),
                           ms_per_step=1e3 * e2e_s, steps=e2e_steps) if e2e_s else

@@ -83,6 +83,8 @@ typedef struct trd_config {
     double sd_c0, sd_c2;             /* sigma_dydx(s)         (res_model = 1) */
     double sin_lorentz;              /* optimum of both polynomials, sin of the Lorentz angle (about +-8 degrees) */
     double tan_tilt;                 /* tan of the pad tilt (2 degrees) */
+    double x_ref;                    /* trd_refit: local x of the reference plane (247: the TPC outer wall of the configs) */
+    double refit_var[5];             /* trd_refit: variances the covariance is reset to (y, z, sin(phi), tan(lambda), q/pT) */
 } trd_config;
 
 /* Input tracks of one batch: device pointers, each of length n_tracks. */
@@ -112,6 +114,16 @@ typedef struct trd_tracks_out {
     int32_t* n_matched;
     int32_t* n_cand_evals;
 } trd_tracks_out;
+
+/* Output of trd_refit: caller-allocated device pointers, each of length n_tracks. */
+typedef struct trd_refit_out {
+    float* par[5];
+    float* cov[15];
+    float* x;           /* x_ref for a refitted track */
+    int32_t* sector;
+    float* chi2;        /* sum of the chi2 increments of the refit */
+    int32_t* n_used;    /* tracklets used; 0 = not refitted, the matcher's state was copied through */
+} trd_refit_out;
 
 /* What trd_load_tracklets built (for tests and traffic accounting). */
 typedef struct trd_index_info {
@@ -168,6 +180,15 @@ int trd_set_chamber_dx(trd_handle* h, const float* dx, int32_t n_chambers, void*
 /* The tracking step for one batch (n_tracks >= 0) against the loaded index. */
 int trd_match(trd_handle* h, const trd_tracks_in* in, const trd_tracks_out* out, int64_t n_tracks,
               void* stream);
+
+/* TRD-only refit of the matched chains (calibration step 3: refits "ignoring the TPC clusters";
+ * PAPER.md:9): for every track with at least two attached tracklets the matcher's final state is taken
+ * as the starting point, its covariance is reset to diag(refit_var), the Kalman filter runs INWARD over the attached
+ * tracklets only (same propagation, sector rule and measurement model as trd_match) and the result is propagated
+ * to x_ref.  `matched` is what trd_match wrote (device arrays; the tracklets it refers to must still be the loaded
+ * ones); a tracklet attached in another sector frame than the state's is skipped; tracks that cannot be refitted
+ * are copied through with n_used = 0.  out->par etc. may alias matched->par etc. */
+int trd_refit(trd_handle* h, const trd_tracks_out* matched, const trd_refit_out* out, int64_t n_tracks, void* stream);
 
 /* The same two calls with HOST arrays (pinned memory makes the copies asynchronous; pageable memory works
  * too).  The library stages through its own device buffers and pipelines on two internal copy streams:

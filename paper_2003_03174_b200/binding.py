@@ -20,7 +20,7 @@ TRD_MAX_HYP = 8
 TRD_OK, TRD_E_ARG, TRD_E_CUDA, TRD_E_NOMEM, TRD_E_STATE = 0, -1, -2, -3, -4
 _STATUS = {0: "TRD_OK", -1: "TRD_E_ARG", -2: "TRD_E_CUDA", -3: "TRD_E_NOMEM", -4: "TRD_E_STATE"}
 
-EXPORTS = ("trd_version", "trd_create", "trd_destroy", "trd_load_tracklets", "trd_load_tracklets_tf", "trd_set_chamber_dx", "trd_match",
+EXPORTS = ("trd_version", "trd_create", "trd_destroy", "trd_load_tracklets", "trd_load_tracklets_tf", "trd_set_chamber_dx", "trd_match", "trd_refit",
            "trd_load_tracklets_host", "trd_match_host", "trd_match_host_async", "trd_wait_host", "trd_get_index_info", "trd_copy_index",
            "trd_last_error", "trd_device_bytes", "trd_kernel_launches", "trd_last_match_kernel_ms")
 
@@ -37,7 +37,10 @@ class TrdConfig(C.Structure):
                 ("chi2_penalty", C.c_double), ("max_snp", C.c_double), ("ybin_width", C.c_double),
                 ("track_binning", C.c_int32), ("res_model", C.c_int32),
                 ("sy_c0", C.c_double), ("sy_c2", C.c_double), ("sd_c0", C.c_double), ("sd_c2", C.c_double),
-                ("sin_lorentz", C.c_double), ("tan_tilt", C.c_double)]
+                ("sin_lorentz", C.c_double), ("tan_tilt", C.c_double), ("x_ref", C.c_double),
+                ("refit_var", C.c_double * 5)]
+
+REFIT_VAR = (1.0, 25.0, 2.5e-3, 2.5e-3, 0.25)     # default reset variances of trd_refit (R31)
 
 
 class TrdTracksIn(C.Structure):
@@ -49,6 +52,11 @@ class TrdTracksOut(C.Structure):
     _fields_ = [("tracklet_idx", C.c_void_p * TRD_MAX_LAYERS), ("par", C.c_void_p * 5), ("cov", C.c_void_p * 15),
                 ("x", C.c_void_p), ("sector", C.c_void_p), ("chi2", C.c_void_p), ("n_matched", C.c_void_p),
                 ("n_cand_evals", C.c_void_p)]
+
+
+class TrdRefitOut(C.Structure):
+    _fields_ = [("par", C.c_void_p * 5), ("cov", C.c_void_p * 15), ("x", C.c_void_p), ("sector", C.c_void_p),
+                ("chi2", C.c_void_p), ("n_used", C.c_void_p)]
 
 
 class TrdIndexInfo(C.Structure):
@@ -89,6 +97,7 @@ def lib():
                                             C.c_int64, C.c_void_p]
         l.trd_set_chamber_dx.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]
         l.trd_match.argtypes = [C.c_void_p, C.POINTER(TrdTracksIn), C.POINTER(TrdTracksOut), C.c_int64, C.c_void_p]
+        l.trd_refit.argtypes = [C.c_void_p, C.POINTER(TrdTracksOut), C.POINTER(TrdRefitOut), C.c_int64, C.c_void_p]
         l.trd_match_host.argtypes = l.trd_match.argtypes
         l.trd_match_host_async.argtypes = l.trd_match.argtypes
         l.trd_wait_host.argtypes = [C.c_void_p, C.c_void_p]
@@ -120,6 +129,9 @@ def make_config(cfg: dict) -> TrdConfig:
     c.res_model = int(cfg.get("res_model", 0))
     for k in ("sy_c0", "sy_c2", "sd_c0", "sd_c2", "sin_lorentz", "tan_tilt"):
         setattr(c, k, float(cfg.get(k, 0.0)))
+    c.x_ref = float(cfg.get("x_ref", 247.0))
+    for i, v in enumerate(cfg.get("refit_var", REFIT_VAR)):
+        c.refit_var[i] = float(v)
     return c
 
 
@@ -229,6 +241,33 @@ def trd_match(h, tracks: dict, out: Optional[dict] = None, n_tracks: Optional[in
         tout.n_matched = _dev_ptr(out["n_matched"], "i32", n)
         tout.n_cand_evals = _dev_ptr(out["n_evals"], "i32", n) if "n_evals" in out else None
     _check(h, lib().trd_match(h, C.byref(tin), C.byref(tout), n, _stream(stream)))
+    return out
+
+
+def trd_refit(h, matched: dict, out: Optional[dict] = None, stream=None) -> dict:
+    """TRD-only inward refit of the chains in `matched` (the dict trd_match returned, CUDA tensors) to the plane
+    x_ref.  Returns par (5, n), cov (15, n), x, sector, chi2, n_used as CUDA tensors."""
+    import torch
+    n = matched["x"].numel()
+    dev = matched["x"].device
+    if out is None:
+        out = dict(par=torch.empty((5, n), dtype=torch.float32, device=dev), cov=torch.empty((15, n), dtype=torch.float32, device=dev),
+                   x=torch.empty(n, dtype=torch.float32, device=dev), sector=torch.empty(n, dtype=torch.int32, device=dev),
+                   chi2=torch.empty(n, dtype=torch.float32, device=dev), n_used=torch.empty(n, dtype=torch.int32, device=dev))
+    tm, to = TrdTracksOut(), TrdRefitOut()
+    if n > 0:
+        tm.tracklet_idx[:] = _row_ptrs(matched["idx"], TRD_MAX_LAYERS, n, "i32")
+        tm.par[:] = _row_ptrs(matched["par"], 5, n, "f32")
+        tm.cov[:] = _row_ptrs(matched["cov"], 15, n, "f32")
+        tm.x = _dev_ptr(matched["x"], "f32", n)
+        tm.sector = _dev_ptr(matched["sector"], "i32", n)
+        to.par[:] = _row_ptrs(out["par"], 5, n, "f32")
+        to.cov[:] = _row_ptrs(out["cov"], 15, n, "f32")
+        to.x = _dev_ptr(out["x"], "f32", n)
+        to.sector = _dev_ptr(out["sector"], "i32", n)
+        to.chi2 = _dev_ptr(out["chi2"], "f32", n)
+        to.n_used = _dev_ptr(out["n_used"], "i32", n)
+    _check(h, lib().trd_refit(h, C.byref(tm), C.byref(to), n, _stream(stream)))
     return out
 
 

@@ -63,6 +63,9 @@ bool derive_params(const trd_config& c, trd::MatchParams& mp) {
     mp.sd_c2 = (float)c.sd_c2;
     mp.sin_lorentz = (float)c.sin_lorentz;
     mp.tan_tilt = (float)c.tan_tilt;
+    mp.tan_half = (float)tan(half);
+    mp.x_ref = (float)c.x_ref;
+    for (int k = 0; k < 5; ++k) mp.refit_var[k] = (float)c.refit_var[k];
     return true;
 }
 
@@ -198,6 +201,27 @@ int trd_set_chamber_dx(trd_handle* h, const float* dx, int32_t n_chambers, void*
     if (e != cudaSuccess) return fail_cuda(h, e, "trd_set_chamber_dx");
     h->mp.dx_max = mx;
     h->index_loaded = false;                             // the next trd_load_tracklets picks the offsets up
+    return TRD_OK;
+}
+
+int trd_refit(trd_handle* h, const trd_tracks_out* m, const trd_refit_out* out, int64_t n, void* stream) {
+    if (!h) return TRD_E_ARG;
+    if (!m || !out || n < 0) return fail(h, TRD_E_ARG, "trd_refit: NULL struct or negative n_tracks");
+    if (!h->index_loaded) return fail(h, TRD_E_STATE, "trd_refit: no tracklets loaded");
+    if (!(h->cfg.x_ref > 0.0)) return fail(h, TRD_E_ARG, "trd_refit: trd_config.x_ref must be positive");
+    for (int k = 0; k < 5; ++k)
+        if (!(h->cfg.refit_var[k] > 0.0)) return fail(h, TRD_E_ARG, "trd_refit: trd_config.refit_var must be positive");
+    if (n == 0) return TRD_OK;
+    for (int k = 0; k < 5; ++k)
+        if (!m->par[k] || !out->par[k]) return fail(h, TRD_E_ARG, "trd_refit: NULL par array");
+    for (int k = 0; k < 15; ++k)
+        if (!m->cov[k] || !out->cov[k]) return fail(h, TRD_E_ARG, "trd_refit: NULL cov array");
+    for (int l = 0; l < TRD_MAX_LAYERS; ++l)
+        if (!m->tracklet_idx[l]) return fail(h, TRD_E_ARG, "trd_refit: NULL tracklet_idx array");
+    if (!m->x || !m->sector || !out->x || !out->sector || !out->chi2 || !out->n_used)
+        return fail(h, TRD_E_ARG, "trd_refit: NULL array");
+    const cudaError_t e = trd::launch_refit(h, *m, *out, n, (cudaStream_t)stream);
+    if (e != cudaSuccess) return fail_cuda(h, e, "trd_refit");
     return TRD_OK;
 }
 

@@ -52,6 +52,9 @@ struct MatchParams {
     float n_sigma_angle, sy_c0, sy_c2, sd_c0, sd_c2, sin_lorentz, tan_tilt;
     // two-stage propagation: largest |radial chamber offset|, 0 = all chambers on their nominal plane
     float dx_max;
+    // trd_refit
+    float tan_half;                  // tan(pi / n_sectors): sector edge in y = x * tan_half
+    float x_ref, refit_var[5];
 };
 
 struct Buffer {
@@ -114,6 +117,8 @@ cudaError_t build_index(trd_handle* h, const float* d_y, const float* d_z, const
                         const int32_t* d_chamber, const int32_t* d_interaction, int n_interactions, int64_t n,
                         cudaStream_t stream);
 cudaError_t launch_match(trd_handle* h, const trd_tracks_in& in, const trd_tracks_out& out, int64_t n,
+                         cudaStream_t stream);
+cudaError_t launch_refit(trd_handle* h, const trd_tracks_out& matched, const trd_refit_out& out, int64_t n,
                          cudaStream_t stream);
 
 // packed track records used when a batch is binned before matching (tracks.cu, match.cu)
