@@ -330,8 +330,9 @@ def test_two_stage_propagation_with_displaced_chambers(B, name, n_hyp, extra):
     d = W.generate(spec); cfg = W.matcher_config(spec)
     want = O.match(cfg, d)
     got = run_gpu(B, cfg, d)
-    assert_parity(P.compare(got, want, x_atol=1e-4), want)
-    assert_parity(P.compare(run_gpu(B, dict(cfg, track_binning=1), d, batch=1999), want, x_atol=1e-4), want)
+    # one more float32 propagation per attached tracklet: the absolute floor of the stress sweep
+    assert_parity(P.compare(got, want, x_atol=1e-4, par_atol=3e-5), want)
+    assert_parity(P.compare(run_gpu(B, dict(cfg, track_binning=1), d, batch=1999), want, x_atol=1e-4, par_atol=3e-5), want)
     assert np.abs(got["x"] - 364.0).max() > 0.3                       # states live at the displaced radii
     # the offsets matter, and clearing them gives the plain matcher again
     plain_want = O.match(cfg, {k: v for k, v in d.items() if k != "chamber_dx"})
