@@ -168,7 +168,7 @@ def run_ours(args, spec, cfg):
     rank, world, local = D.env_rank()
     torch.cuda.set_device(local)
     device = torch.device("cuda", local)
-    D.init("nccl")
+    D.init("nccl", device)
     if rank == 0:
         Bd.build()
     D.barrier()

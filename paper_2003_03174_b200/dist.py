@@ -15,15 +15,17 @@ def env_rank() -> Tuple[int, int, int]:
     return (int(os.environ.get("RANK", 0)), int(os.environ.get("WORLD_SIZE", 1)), int(os.environ.get("LOCAL_RANK", 0)))
 
 
-def init(backend: str):
-    """Initialise torch.distributed from the environment if WORLD_SIZE > 1.  Returns (rank, world)."""
+def init(backend: str, device=None):
+    """Initialise torch.distributed from the torchrun environment (also for a single rank, so that the same
+    barrier / all-reduce code runs at every N).  Returns (rank, world)."""
     rank, world, _ = env_rank()
-    if world > 1:
+    if world > 1 or "TORCHELASTIC_RUN_ID" in os.environ:
         import torch.distributed as dist
         if not dist.is_initialized():
             os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
             os.environ.setdefault("MASTER_PORT", "29500")
-            dist.init_process_group(backend=backend, rank=rank, world_size=world)
+            kw = dict(device_id=device) if (device is not None and backend == "nccl") else {}
+            dist.init_process_group(backend=backend, rank=rank, world_size=world, **kw)
     return rank, world
 
 
