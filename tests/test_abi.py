@@ -80,3 +80,38 @@ def test_product_path_does_not_reach_the_oracle():
             if f.endswith((".py", ".cu", ".cuh", ".h")):
                 text = open(os.path.join(dp, f)).read()
                 assert "from oracle" not in text and "import oracle" not in text and "trd_oracle" not in text, f
+
+
+def test_plain_c_program_links_and_calls_the_library(lib):
+    """A C99 program (no Python, no torch) links against libtrdmatch.so and uses the ABI: version, argument
+    errors, and -- on a machine without a GPU -- the loud TRD_E_CUDA from trd_create."""
+    src = r'''
+#include "trdmatch.h"
+#include <stdio.h>
+#include <string.h>
+int main(void) {
+    trd_config c; trd_handle* h = 0;
+    memset(&c, 0, sizeof c);
+    if (trd_version() != TRD_VERSION) return 1;
+    if (trd_create(0, &h) != TRD_E_ARG) return 2;
+    c.struct_size = sizeof c;                       /* all other fields 0: invalid geometry */
+    if (trd_create(&c, &h) != TRD_E_ARG || h != 0) return 3;
+    c.n_sectors = 18; c.n_stacks = 5; c.n_layers = 6; c.n_hyp = 4;
+    { double x[6] = {300, 313, 326, 338, 351, 364}; memcpy(c.layer_x, x, sizeof x); }
+    c.z_max = 350; c.pad_length = 8; c.bz_tesla = 0.5; c.sigma_y = 0.04; c.sigma_z = 2.3094; c.sigma_dydx = 0.02;
+    c.n_sigma_road = 3; c.n_sigma_angle = 4; c.chi2_cut = 15; c.chi2_penalty = 15; c.max_snp = 0.95;
+    { int rc = trd_create(&c, &h); printf("%d\n", rc); if (rc == TRD_OK) { trd_destroy(h); } else if (rc != TRD_E_CUDA) return 4; }
+    trd_destroy(0);
+    return 0;
+}
+'''
+    with tempfile.TemporaryDirectory() as td:
+        cfile = os.path.join(td, "t.c"); exe = os.path.join(td, "t")
+        open(cfile, "w").write(src)
+        libdir = os.path.dirname(Bd.LIB_PATH)
+        subprocess.check_call(["gcc", "-std=c99", "-Wall", "-Werror", "-I", os.path.join(ROOT, "include"), cfile, "-o", exe,
+                               "-L", libdir, "-ltrdmatch", "-Wl,-rpath," + libdir])
+        out = subprocess.run([exe], capture_output=True, text=True)
+    assert out.returncode == 0, (out.returncode, out.stdout, out.stderr)
+    import torch
+    assert int(out.stdout.split()[0]) == (B.TRD_OK if torch.cuda.is_available() else B.TRD_E_CUDA)
