@@ -196,8 +196,8 @@ int trd_refit(trd_handle* h, const trd_tracks_out* matched, const trd_refit_out*
  *   trd_load_tracklets_host   returns once the copies and kernels are queued; the arrays must stay valid
  *                             until trd_wait_host has returned;
  *   trd_match_host_async      queues copy-in, trd_match and copy-out of one batch and returns; the results
- *                             are in `out_host` only after trd_wait_host.  At most two batches are in flight:
- *                             a third call first waits for the oldest;
+ *                             are in `out_host` only after trd_wait_host.  At most four batches are in flight:
+ *                             a fifth call first waits for the oldest;
  *   trd_wait_host             blocks until everything queued by *_host calls has completed;
  *   trd_match_host            = trd_match_host_async + trd_wait_host. */
 int trd_load_tracklets_host(trd_handle* h, const float* y, const float* z, const float* dydx,

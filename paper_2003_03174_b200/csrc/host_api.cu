@@ -1,6 +1,6 @@
 // host_api.cu -- the *_host entry points of include/trdmatch.h: staging and copy/compute overlap.
 // Three streams: s_in (host->device copies), the caller's stream (all kernels), s_out (device->host
-// copies), chained by events.  Tracks use a ring of two staging slots so that the copy-in of batch k+1 and
+// copies), chained by events.  Tracks use a ring of four staging slots so that the copy-in of batch k+1 and
 // the copy-out of batch k-1 run while batch k is matched.  No arithmetic of the method lives here.
 #include "trd_internal.cuh"
 

@@ -93,7 +93,7 @@ struct trd_handle {
     // staging for the *_host entry points
     trd::Buffer stage_tl;   // tracklets
     // pipelined host entry points (host_api.cu): own copy streams, a ring of staging slots
-    static constexpr int kRing = 2;
+    static constexpr int kRing = 4;
     cudaStream_t s_in = nullptr, s_out = nullptr;        // host->device and device->host copy streams
     trd::Buffer stage_in[kRing], stage_out[kRing];       // tracks in / out per ring slot
     cudaEvent_t ev_in[kRing] = {}, ev_done[kRing] = {}, ev_out[kRing] = {};   // copied in / matched / copied out

@@ -228,13 +228,13 @@ def test_track_binning_does_not_change_results(B, name):
 
 
 def test_pipelined_host_entry_points(B):
-    """trd_match_host_async + trd_wait_host: five batches through the two-slot ring (the third call has to
+    """trd_match_host_async + trd_wait_host: nine batches through the four-slot ring (the fifth call has to
     retire the first), pinned and pageable buffers, two consecutive loads on one handle; bit-equal to the
     device entry points."""
     spec = W.CONFIGS["pileup"]; d = W.generate(spec); cfg = dict(W.matcher_config(spec), track_binning=1)
     want = run_gpu(B, cfg, d)
     n = spec.n_tracks
-    bounds = [(lo, min(n, lo + 5003)) for lo in range(0, n, 5003)]
+    bounds = [(lo, min(n, lo + 2801)) for lo in range(0, n, 2801)]
     h = B.trd_create(cfg)
     try:
         for pinned in (True, False):
