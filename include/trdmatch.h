@@ -219,6 +219,9 @@ int64_t trd_kernel_launches(const trd_handle* h); /* kernels launched through th
 /* Device time of the match kernel alone in the most recent trd_match (CUDA events recorded on the call's
  * stream around that one launch; waits for the end event).  TRD_E_STATE if no trd_match has run. */
 int trd_last_match_kernel_ms(trd_handle* h, float* ms);
+/* The same for the n most recent trd_match calls (n <= 64; ms[n - 1] is the latest): the library keeps a ring of event
+ * pairs, so a timed loop can run without any synchronisation and be read afterwards. */
+int trd_match_kernel_ms(trd_handle* h, float* ms, int32_t n);
 
 #ifdef __cplusplus
 }

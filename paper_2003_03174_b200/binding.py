@@ -22,7 +22,7 @@ _STATUS = {0: "TRD_OK", -1: "TRD_E_ARG", -2: "TRD_E_CUDA", -3: "TRD_E_NOMEM", -4
 
 EXPORTS = ("trd_version", "trd_create", "trd_destroy", "trd_load_tracklets", "trd_load_tracklets_tf", "trd_set_chamber_dx", "trd_match", "trd_refit",
            "trd_load_tracklets_host", "trd_match_host", "trd_match_host_async", "trd_wait_host", "trd_get_index_info", "trd_copy_index",
-           "trd_last_error", "trd_device_bytes", "trd_kernel_launches", "trd_last_match_kernel_ms")
+           "trd_last_error", "trd_device_bytes", "trd_kernel_launches", "trd_last_match_kernel_ms", "trd_match_kernel_ms")
 
 _fp = C.POINTER(C.c_float)
 _ip = C.POINTER(C.c_int32)
@@ -110,6 +110,7 @@ def lib():
         l.trd_kernel_launches.argtypes = [C.c_void_p]
         l.trd_kernel_launches.restype = C.c_int64
         l.trd_last_match_kernel_ms.argtypes = [C.c_void_p, C.POINTER(C.c_float)]
+        l.trd_match_kernel_ms.argtypes = [C.c_void_p, C.POINTER(C.c_float), C.c_int32]
         _lib = l
     return _lib
 
@@ -357,6 +358,13 @@ def trd_device_bytes(h) -> int:
 
 def trd_kernel_launches(h) -> int:
     return int(lib().trd_kernel_launches(h))
+
+
+def trd_match_kernel_ms(h, n: int) -> list:
+    """Device times [ms] of the match kernel in the n most recent trd_match calls (n <= 64), oldest first."""
+    ms = (C.c_float * n)()
+    _check(h, lib().trd_match_kernel_ms(h, ms, n))
+    return [float(v) for v in ms]
 
 
 def trd_last_match_kernel_ms(h) -> float:

@@ -153,8 +153,9 @@ void trd_destroy(trd_handle* h) {
     }
     release(h->trk_hist);
     release(h->trk_tot);
-    for (int k = 0; k < 2; ++k)
-        if (h->ev_match[k]) cudaEventDestroy(h->ev_match[k]);
+    for (int r = 0; r < trd_handle::kEvRing; ++r)
+        for (int k = 0; k < 2; ++k)
+            if (h->ev_match[r][k]) cudaEventDestroy(h->ev_match[r][k]);
     delete h;
 }
 
@@ -288,13 +289,18 @@ int64_t trd_device_bytes(const trd_handle* h) {
 
 int64_t trd_kernel_launches(const trd_handle* h) { return h ? h->launches : 0; }
 
-int trd_last_match_kernel_ms(trd_handle* h, float* ms) {
-    if (!h || !ms) return TRD_E_ARG;
-    if (!h->ev_recorded) return fail(h, TRD_E_STATE, "trd_last_match_kernel_ms: no trd_match has run");
-    cudaError_t e = cudaEventSynchronize(h->ev_match[1]);
-    if (e == cudaSuccess) e = cudaEventElapsedTime(ms, h->ev_match[0], h->ev_match[1]);
-    if (e != cudaSuccess) return fail_cuda(h, e, "trd_last_match_kernel_ms");
+int trd_match_kernel_ms(trd_handle* h, float* ms, int32_t n) {
+    if (!h || !ms || n < 1) return TRD_E_ARG;
+    if (n > trd_handle::kEvRing || n > h->ev_count) return fail(h, TRD_E_STATE, "trd_match_kernel_ms: fewer trd_match calls on record");
+    for (int k = 0; k < n; ++k) {                     // ms[n - 1] is the most recent call
+        cudaEvent_t* ev = h->ev_match[(h->ev_count - n + k) % trd_handle::kEvRing];
+        cudaError_t e = cudaEventSynchronize(ev[1]);
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms[k], ev[0], ev[1]);
+        if (e != cudaSuccess) return fail_cuda(h, e, "trd_match_kernel_ms");
+    }
     return TRD_OK;
 }
+
+int trd_last_match_kernel_ms(trd_handle* h, float* ms) { return trd_match_kernel_ms(h, ms, 1); }
 
 }  // extern "C"

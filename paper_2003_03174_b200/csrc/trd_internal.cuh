@@ -75,8 +75,9 @@ struct trd_handle {
     int key_bits = 0, n_passes = 0;
     double ybin_width = 0.0;
     int64_t launches = 0;
-    cudaEvent_t ev_match[2] = {nullptr, nullptr};   // around the match kernel of the last trd_match
-    bool ev_recorded = false;
+    static constexpr int kEvRing = 64;               // event pairs around the match kernels of the last 64 trd_match calls
+    cudaEvent_t ev_match[kEvRing][2] = {};
+    int64_t ev_count = 0;                            // trd_match calls that recorded events so far
     std::string err;
     // device buffers owned by the handle
     trd::Buffer store;      // float4 per sorted tracklet: y, z, dy/dx, original position (bits)
