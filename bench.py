@@ -372,6 +372,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--interactions", type=int, default=0,
                     help="> 1: time-frame association with this many interactions (SURVEY.md 8(f) NEXT#2)")
+    ap.add_argument("--ybin-width", type=float, default=0.0, help="local-y bin width of the index in cm (0 = chosen by the library)")
     ap.add_argument("--chamber-dx", type=float, default=0.0,
                     help="> 0: chambers displaced radially by N(0, this) cm, two-stage propagation (SURVEY.md 8(f) NEXT#3)")
     ap.add_argument("--res-model", type=int, default=0, choices=[0, 1],
@@ -389,6 +390,8 @@ def main():
     if args.chamber_dx > 0.0:
         spec = dataclasses.replace(spec, chamber_dx_sigma=args.chamber_dx, name=spec.name + "_dx")
     cfg = W.matcher_config(spec)
+    if args.ybin_width > 0.0:
+        cfg["ybin_width"] = args.ybin_width
     if args.impl == "reference":
         run_reference(args, spec, cfg)
     else:
