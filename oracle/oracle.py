@@ -19,6 +19,7 @@ _LIB = os.path.join(_HERE, "build", "libtrd_oracle.so")
 _lib = None
 
 N_LAYERS_MAX = 6
+PION_MASS = 0.13957                                # GeV: the mass hypothesis of the material corrections [R33]
 REFIT_VAR = (1.0, 25.0, 2.5e-3, 2.5e-3, 0.25)     # default reset variances of the TRD-only refit [R31]
 
 
@@ -33,6 +34,7 @@ class OrcConfig(C.Structure):
         ("sy_c0", C.c_double), ("sy_c2", C.c_double), ("sd_c0", C.c_double), ("sd_c2", C.c_double),
         ("sin_lorentz", C.c_double), ("tan_tilt", C.c_double), ("res_model", C.c_int32), ("pad_", C.c_int32),
         ("x_ref", C.c_double), ("refit_var", C.c_double * 5),
+        ("x_over_x0", C.c_double), ("eloss", C.c_double), ("eloss_fluct", C.c_double), ("mass", C.c_double),
     ]
 
 
@@ -72,6 +74,10 @@ def make_config(cfg: dict) -> OrcConfig:
     c.x_ref = float(cfg.get("x_ref", 247.0))
     for i, v in enumerate(cfg.get("refit_var", REFIT_VAR)):
         c.refit_var[i] = float(v)
+    # material in front of every layer [R32, R33]; absent = none
+    for k in ("x_over_x0", "eloss", "eloss_fluct"):
+        setattr(c, k, float(cfg.get(k, 0.0)))
+    c.mass = float(cfg.get("mass", PION_MASS))
     return c
 
 
@@ -130,6 +136,13 @@ def update(cfg: dict, p, c15, ym, zm, layer: int = 0):
     p = np.array(p, float); c15 = np.array(c15, float)
     chi2 = lib().orc_update(C.byref(make_config(cfg)), _dp(p), _dp(c15), C.c_double(ym), C.c_double(zm), int(layer))
     return p, c15, float(chi2)
+
+
+def material(cfg: dict, p, c15, direction: int = 1):
+    """One slab of material at the current point (direction +1 outward, -1 inward).  Returns (ok, p, c15)."""
+    p = np.array(p, float); c15 = np.array(c15, float)
+    ok = lib().orc_material(C.byref(make_config(cfg)), _dp(p), _dp(c15), int(direction))
+    return bool(ok), p, c15
 
 
 def road(cfg: dict, p, c15, layer: int = 0):

@@ -55,6 +55,10 @@ struct Config {
     int32_t res_model, pad_;
     // TRD-only refit (PAPER.md:33 step 3) [R31]: reference plane and the variances the covariance is reset to
     double x_ref, refit_var[5];
+    // material in front of every layer plane ("taking into account ... energy loss") [R32, R33]:
+    // thickness in radiation lengths and mean energy loss [GeV] at normal incidence and beta = 1, relative width of
+    // the energy-loss fluctuation, particle mass [GeV].  All zero = no material (the configs).
+    double x_over_x0, eloss, eloss_fluct, mass;
 };
 
 struct Hyp {
@@ -205,6 +209,50 @@ bool rotate(const Config& cfg, Hyp& h, double beta, double* margin, Counters* cn
     std::memcpy(h.p, out, sizeof out);
     similarity(J, h.C);
     h.x = xn;
+    return true;
+}
+
+// ---- material: a thin slab crossed at the current point ("energy loss and
+// multiple scattering as process noise", C' = F C F^T + Q) [R32, R33].  dir = +1 going outward (the particle loses
+// energy), -1 going inward (the refit runs against the flight direction and gives the energy back).
+//   path factor      ell = sqrt((1 + t^2) / (1 - s^2))          (slab normal to the local x axis)
+//   momentum         p = sqrt(1 + t^2) / |c|,  E = sqrt(p^2 + m^2),  beta = p / E
+//   scattering       theta0 = 0.0136 GeV / (beta p) sqrt(x/X0 ell)   (Highland's width without the log term)
+//                    two independent angles: theta1 changes lambda, theta2 / cos(lambda) changes phi, |p| stays:
+//                    ds = sqrt(1 - s^2) sqrt(1 + t^2) theta2,  dt = (1 + t^2) theta1,  dc = c t theta1
+//                    Q_ss = th0^2 (1 - s^2)(1 + t^2), Q_tt = th0^2 (1 + t^2)^2, Q_tc = th0^2 c t (1 + t^2), Q_cc = th0^2 c^2 t^2
+//   energy loss      dE = eloss ell / beta^2,  E' = E - dir dE,  p' = sqrt(E'^2 - m^2),  c' = c p / p'  (direction kept);
+//                    fluctuation sigma_E = eloss_fluct dE, d(c)/dE = c E / p^2:  Q_cc += (c E / p^2 sigma_E)^2
+// Position and covariance of (y, z) are untouched (thin slab); the covariance gets only the additive Q (the
+// Jacobian of the mean energy-loss correction, 1 + O(dE / E), is neglected).  Returns false if the particle stops.
+inline bool has_material(const Config& cfg) { return cfg.x_over_x0 > 0.0 || cfg.eloss > 0.0; }
+
+bool apply_material(const Config& cfg, Hyp& h, int dir, double* margin) {
+    const double s = h.p[2], t = h.p[3], c = h.p[4];
+    if (c == 0.0 || std::fabs(s) >= 1.0) return true;           // infinite momentum: nothing happens
+    const double ell = std::sqrt((1.0 + t * t) / (1.0 - s * s));
+    const double p2 = (1.0 + t * t) / (c * c);
+    const double e2 = p2 + cfg.mass * cfg.mass;
+    const double beta2 = p2 / e2;
+    const double E = std::sqrt(e2);
+    const double dE = cfg.eloss * ell / beta2;
+    const double E1 = E - dir * dE;
+    if (dE > 0.0) {
+        note(margin, E1, cfg.mass);
+        if (E1 <= cfg.mass) return false;                       // stopped in the slab: state untouched
+    }
+    const double th2 = 0.0136 * 0.0136 * cfg.x_over_x0 * ell / (beta2 * p2);
+    h.C[2][2] += th2 * (1.0 - s * s) * (1.0 + t * t);
+    h.C[3][3] += th2 * (1.0 + t * t) * (1.0 + t * t);
+    h.C[3][4] += th2 * c * t * (1.0 + t * t);
+    h.C[4][3] = h.C[3][4];
+    h.C[4][4] += th2 * c * c * t * t;
+    if (dE > 0.0) {
+        const double sigE = cfg.eloss_fluct * dE;
+        const double dcdE = c * E / p2;
+        h.C[4][4] += dcdE * dcdE * sigE * sigE;
+        h.p[4] = c * std::sqrt(p2 / (E1 * E1 - cfg.mass * cfg.mass));
+    }
     return true;
 }
 
@@ -415,6 +463,7 @@ void match_track(const Config& cfg, const Store& st, const Hyp& seed, TrackResul
         for (int ih = 0; ih < (int)hyps.size(); ++ih) {
             Hyp& h = prop[ih];
             if (h.alive) h.alive = propagate_to_layer(cfg, h, cfg.layer_x[L], mg, cnt);
+            if (h.alive && has_material(cfg)) h.alive = apply_material(cfg, h, +1, mg);   // the slab in front of the plane [R32]
             if (h.alive) {
                 const Road rd = make_road(cfg, h, L);
                 if (cnt) cnt->n_road++;
@@ -538,6 +587,16 @@ int orc_propagate_to_layer(const orc_config* cfg, double p[5], double c15[15], d
     store_cov(h, c15);
     *x = h.x;
     *sector = h.sector;
+    return 1;
+}
+
+// one slab of material at the current point, dir = +1 outward / -1 inward; returns 0 if the particle stops
+int orc_material(const orc_config* cfg, double p[5], double c15[15], int dir) {
+    Hyp h;
+    load_hyp(h, p, c15, 0.0, 0);
+    if (!apply_material(*cfg, h, dir, nullptr)) return 0;
+    std::memcpy(p, h.p, sizeof h.p);
+    store_cov(h, c15);
     return 1;
 }
 
@@ -670,17 +729,27 @@ int orc_refit(const orc_config* cfg, const float* tl_y, const float* tl_z, const
         if (ok) {
             for (int a = 0; a < 5; ++a)
                 for (int b = 0; b < 5; ++b) h.C[a][b] = (a == b) ? cfg->refit_var[a] : 0.0;
+            // With material [R34] every layer plane from the outermost attached tracklet inward is a stop: the plane of
+            // the attached tracklet (exact radius) or the nominal one, then the slab in front of it is crossed inward
+            // (noise added, mean energy loss given back) before the next step.  Slabs outside the outermost attached
+            // tracklet are not applied: the covariance is reset there anyway.
+            const bool mat = has_material(*cfg);
+            bool started = false;
             for (int l = cfg->n_layers - 1; l >= 0 && ok; --l) {
                 const int k = in_idx[l * n_trk + i];
-                if (k < 0 || k >= n_tl) continue;
-                const int ch = tl_chamber[k];
-                const double X = cfg->layer_x[l] + (chamber_dx ? chamber_dx[ch] : 0.0);
+                const bool att = k >= 0 && k < n_tl;
+                if (!att && !(mat && started)) continue;
+                const int ch = att ? tl_chamber[k] : 0;
+                const double X = cfg->layer_x[l] + ((att && chamber_dx) ? chamber_dx[ch] : 0.0);
                 if (h.x != X) ok = propagate_to_layer(*cfg, h, X, nullptr, nullptr);
                 if (!ok) break;
-                if (ch / per_sector != h.sector) continue;           // attached in another frame: not used
-                chi2 += kalman_update(*cfg, h, l, (double)tl_y[k], (double)tl_z[k]);
-                ++n_used;
-                if (std::fabs(h.p[2]) >= cfg->max_snp) ok = false;
+                if (att && ch / per_sector == h.sector) {            // attached in another frame: not used
+                    chi2 += kalman_update(*cfg, h, l, (double)tl_y[k], (double)tl_z[k]);
+                    ++n_used;
+                    if (std::fabs(h.p[2]) >= cfg->max_snp) ok = false;
+                }
+                if (att) started = true;
+                if (ok && mat) ok = apply_material(*cfg, h, -1, nullptr);
             }
             if (ok) ok = propagate_to_layer(*cfg, h, cfg->x_ref, nullptr, nullptr);
         }

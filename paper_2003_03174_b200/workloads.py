@@ -61,6 +61,14 @@ SD_C0, SD_C2 = 0.015, 0.06           # dy/dx: "below 1 degree" at the optimum (P
 LORENTZ_DEG = 8.0
 TILT_DEG = 2.0
 
+# Material of PAPER.md:64 (the ALICE material budget is not available: synthetic, R32/R33).  One slab in
+# front of every layer plane; the values used by the material workloads:
+PION_MASS = 0.13957                  # GeV
+X_OVER_X0 = 0.04                     # radiation lengths per layer at normal incidence
+ELOSS = 1.5e-3                       # GeV per layer at normal incidence and beta = 1
+ELOSS_FLUCT = 0.3                    # relative width of the energy-loss fluctuation
+HIGHLAND = 0.0136                    # GeV: theta0 = HIGHLAND / (beta p) sqrt(x/X0)
+
 
 @dataclasses.dataclass(frozen=True)
 class WorkloadSpec:
@@ -81,6 +89,9 @@ class WorkloadSpec:
     efficiency: float = EFFICIENCY
     res_model: int = 0                # 1: sigma_y(sin phi), sigma_dydx(sin phi) polynomials and +-2 degree pad tilt
     chamber_dx_sigma: float = 0.0     # > 0: radial chamber misalignment N(0, sigma) cm, clipped at 3 sigma
+    x_over_x0: float = 0.0            # > 0: a slab of that many radiation lengths in front of every layer:
+    eloss: float = 0.0                # the true particle is scattered there and loses eloss * path / beta^2 GeV
+    eloss_fluct: float = 0.0          # (Gaussian fluctuation of that relative width)
     n_interactions: int = 0           # > 1: time-frame association: tracks i*n_ia//n_tracks form one
                                       # collision, their tracklets inherit its id, noise tracklets get a random one
 
@@ -120,7 +131,9 @@ def matcher_config(spec: WorkloadSpec) -> dict:
     if spec.res_model:
         extra = dict(res_model=1, sy_c0=SY_C0, sy_c2=SY_C2, sd_c0=SD_C0, sd_c2=SD_C2,
                      sin_lorentz=sin_lorentz(spec.bz), tan_tilt=math.tan(math.radians(TILT_DEG)))
-    return dict(extra, 
+    if spec.x_over_x0 > 0.0 or spec.eloss > 0.0:
+        extra.update(x_over_x0=spec.x_over_x0, eloss=spec.eloss, eloss_fluct=spec.eloss_fluct, mass=PION_MASS)
+    return dict(extra,
         n_sectors=N_SECTORS, n_stacks=N_STACKS, n_layers=N_LAYERS,
         layer_x=list(LAYER_X), z_max=Z_MAX, pad_length=PAD_LENGTH, bz_tesla=spec.bz,
         sigma_y=SIGMA_Y_TRACKLET, sigma_z=PAD_LENGTH / math.sqrt(12.0),
@@ -209,6 +222,49 @@ def _truth_in_sector(phi0, kappa, tanl, x_plane, sec):
     return y, tanl * arc, s1, ok
 
 
+def _cross_from(gx, gy, gz, psi, kappa, tanl, x_plane, sec):
+    """Crossing of the plane local-x = x_plane of sector `sec` by the helix that passes the GLOBAL point (gx, gy, gz)
+    with global azimuth psi, signed curvature kappa and tan(lambda) = tanl: the chord relation of _truth_at_plane
+    written from an arbitrary start point.  Returns y, z, sin(phi) (local), ok."""
+    alpha = (sec + 0.5) * SECTOR_WIDTH
+    ca, sa = np.cos(alpha), np.sin(alpha)
+    x0 = gx * ca + gy * sa
+    y0 = -gx * sa + gy * ca
+    ploc = np.mod(psi - alpha + np.pi, 2.0 * np.pi) - np.pi
+    s0, c0 = np.sin(ploc), np.cos(ploc)
+    d = x_plane - x0
+    s1 = s0 + kappa * d
+    ok = (np.abs(s1) < 1.0) & (c0 > 0.0)
+    s1c = np.where(ok, s1, 0.0)
+    c1 = np.sqrt(1.0 - s1c * s1c)
+    straight = np.abs(kappa) < 1e-12
+    ksafe = np.where(straight, 1.0, kappa)
+    c0s = np.where(c0 > 0, c0, 1.0)
+    y = y0 + np.where(straight, d * s0 / c0s, (c0 - c1) / ksafe)
+    arc = np.where(straight, d / c0s, (np.arcsin(s1c) - ploc) / ksafe)
+    return y, gz + tanl * arc, s1, ok
+
+
+def _cross_with_sector_search(gx, gy, gz, psi, kappa, tanl, x_plane):
+    """_cross_from in the sector whose |y| <= x_plane tan(10 deg): the sector of the start point's azimuth (of the
+    direction, at the origin) and its two neighbours are tried.  Returns sector, y, z, sin(phi), ok."""
+    n = gx.shape[0]
+    at_origin = (gx == 0.0) & (gy == 0.0)
+    az = np.where(at_origin, psi + np.arcsin(np.clip(0.5 * kappa * x_plane, -1.0, 1.0)), np.arctan2(gy, gx))
+    guess = np.floor(np.mod(az, 2.0 * np.pi) / SECTOR_WIDTH).astype(np.int64)
+    out = dict(sec=np.zeros(n, np.int64), y=np.full(n, np.nan), z=np.full(n, np.nan), s=np.full(n, np.nan),
+               ok=np.zeros(n, bool))
+    edge = x_plane * TAN_HALF_SECTOR
+    for d in (0, -1, 1):
+        sec = np.mod(guess + d, N_SECTORS)
+        y, z, s1, reach = _cross_from(gx, gy, gz, psi, kappa, tanl, x_plane, sec)
+        take = reach & (np.abs(y) <= edge) & ~out["ok"]
+        for k, v in (("sec", sec), ("y", y), ("z", z), ("s", s1)):
+            out[k] = np.where(take, v, out[k])
+        out["ok"] |= take
+    return out["sec"], out["y"], out["z"], out["s"], out["ok"]
+
+
 def chamber_offsets(spec: "WorkloadSpec") -> np.ndarray:
     """Radial offset of every chamber from its nominal layer plane (float32 cm), own seeded stream."""
     n_ch = N_SECTORS * N_STACKS * N_LAYERS
@@ -279,8 +335,43 @@ def generate(spec: WorkloadSpec) -> dict:
     sig_y, sig_z, sig_d, sig_ch, sig_lab, sig_lay = [], [], [], [], [], []
     truth_last = np.full((n, 4), np.nan)
     ch_dx = chamber_offsets(spec)
+    material = spec.x_over_x0 > 0.0 or spec.eloss > 0.0
+    if material:
+        # stepped truth: global point, azimuth, tan(lambda), q/pT after the last slab crossed (the origin at first)
+        gx, gy, gz = np.zeros(n), np.zeros(n), np.zeros(n)
+        psi, tl_now, qpt_now, going = phi0.copy(), tanl.copy(), qpt.copy(), np.ones(n, bool)
+        truth_last_par = np.full((5, n), np.nan)
     for lay, xl in enumerate(LAYER_X):
-        secl, yl, zl, sl, okl = _truth_at_plane(phi0, kappa, tanl, xl)
+        if material:
+            # crossing of the nominal plane, then the slab: two scattering angles and the energy loss
+            # (draw order per layer: k1, k2, ke, then the draws of the plain generator)
+            secl, yl, zl, sl, okl = _cross_with_sector_search(gx, gy, gz, psi, kfac * qpt_now, tl_now, xl)
+            okl &= going
+            k1, k2, ke = rng.standard_normal(n), rng.standard_normal(n), rng.standard_normal(n)
+            with np.errstate(invalid="ignore"):
+                sc = np.where(okl, sl, 0.0)
+                path = np.sqrt((1.0 + tl_now ** 2) / (1.0 - sc * sc))
+                mom = np.sqrt(1.0 + tl_now ** 2) / np.abs(qpt_now)
+                en = np.sqrt(mom ** 2 + PION_MASS ** 2)
+                beta = mom / en
+                theta0 = HIGHLAND / (beta * mom) * np.sqrt(spec.x_over_x0 * path)
+                lam = np.arctan(tl_now)
+                alpha_l = (secl + 0.5) * SECTOR_WIDTH
+                psi_new = alpha_l + np.arcsin(sc) + theta0 * k2 / np.cos(lam)
+                lam_new = lam + theta0 * k1
+                en_new = en - spec.eloss * path / beta ** 2 * (1.0 + spec.eloss_fluct * ke)
+                okl &= en_new > PION_MASS
+                mom_new = np.sqrt(np.where(okl, en_new ** 2 - PION_MASS ** 2, 1.0))
+            ca, sa = np.cos(alpha_l), np.sin(alpha_l)
+            yc, zc_ = np.where(okl, yl, 0.0), np.where(okl, zl, 0.0)
+            gx, gy, gz = np.where(okl, xl * ca - yc * sa, gx), np.where(okl, xl * sa + yc * ca, gy), np.where(okl, zc_, gz)
+            psi = np.where(okl, psi_new, psi)
+            tl_now = np.where(okl, np.tan(lam_new), tl_now)
+            qpt_now = np.where(okl, q / (mom_new * np.cos(lam_new)), qpt_now)
+            going = okl
+            sl = np.where(okl, np.sin(psi - alpha_l), np.nan)          # the chamber sees the direction after the slab
+        else:
+            secl, yl, zl, sl, okl = _truth_at_plane(phi0, kappa, tanl, xl)
         u = rng.random(n)
         ny = rng.standard_normal(n)
         nd = rng.standard_normal(n)
@@ -288,13 +379,18 @@ def generate(spec: WorkloadSpec) -> dict:
             present = okl & (np.abs(zl) < Z_MAX) & (np.abs(sl) < MAX_SNP) & (u < spec.efficiency)
         if lay == N_LAYERS - 1:
             truth_last[okl] = np.stack([yl, zl, sl, secl.astype(float)], axis=1)[okl]
+            if material:
+                truth_last_par[:, okl] = np.stack([yl, zl, sl, tl_now, qpt_now])[:, okl]
         idx = np.nonzero(present)[0]
         chamber_l = secl[idx] * (N_STACKS * N_LAYERS) + stack_of_z(pad_row_centre(zl[idx])) * N_LAYERS + lay
         if spec.chamber_dx_sigma > 0.0:
             # the chamber sits at x_l + dx: the tracklet is measured where the particle crosses THAT plane
             yl, zl, sl = yl.copy(), zl.copy(), sl.copy()
-            yd, zd, sd, okd = _truth_in_sector(phi0[idx], kappa[idx], tanl[idx], xl + ch_dx[chamber_l].astype(np.float64),
-                                               secl[idx])
+            xd = xl + ch_dx[chamber_l].astype(np.float64)
+            if material:
+                yd, zd, sd, okd = _cross_from(gx[idx], gy[idx], gz[idx], psi[idx], kfac * qpt_now[idx], tl_now[idx], xd, secl[idx])
+            else:
+                yd, zd, sd, okd = _truth_in_sector(phi0[idx], kappa[idx], tanl[idx], xd, secl[idx])
             assert okd.all()
             yl[idx], zl[idx], sl[idx] = yd, zd, sd
         zc = pad_row_centre(zl[idx])
@@ -352,6 +448,8 @@ def generate(spec: WorkloadSpec) -> dict:
 
     if spec.chamber_dx_sigma > 0.0:
         assoc["chamber_dx"] = ch_dx
+    if material:
+        assoc["truth_last_par"] = truth_last_par
     return dict(
         assoc, spec=spec,
         par=np.ascontiguousarray(par, np.float32), cov=np.ascontiguousarray(cov, np.float32),
