@@ -375,6 +375,8 @@ def main():
     ap.add_argument("--ybin-width", type=float, default=0.0, help="local-y bin width of the index in cm (0 = chosen by the library)")
     ap.add_argument("--chamber-dx", type=float, default=0.0,
                     help="> 0: chambers displaced radially by N(0, this) cm, two-stage propagation (SURVEY.md 8(f) NEXT#3)")
+    ap.add_argument("--material", action="store_true",
+                    help="a slab of material in front of every layer: multiple scattering and energy loss (SURVEY.md 8(f) NEXT#3)")
     ap.add_argument("--res-model", type=int, default=0, choices=[0, 1],
                     help="1: inputs and matcher with the sin(phi)-dependent resolutions and pad tilt (SURVEY.md 8(f) NEXT#1)")
     args = ap.parse_args()
@@ -389,6 +391,8 @@ def main():
         spec = dataclasses.replace(spec, n_interactions=args.interactions, name=spec.name + f"_tf{args.interactions}")
     if args.chamber_dx > 0.0:
         spec = dataclasses.replace(spec, chamber_dx_sigma=args.chamber_dx, name=spec.name + "_dx")
+    if args.material:
+        spec = dataclasses.replace(spec, x_over_x0=W.X_OVER_X0, eloss=W.ELOSS, eloss_fluct=W.ELOSS_FLUCT, name=spec.name + "_mat")
     cfg = W.matcher_config(spec)
     if args.ybin_width > 0.0:
         cfg["ybin_width"] = args.ybin_width

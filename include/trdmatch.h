@@ -7,7 +7,7 @@
  * inclination is more than n_sigma_angle sigma off the track inclination are excluded
  * (PAPER.md:60), the best n_hyp hypotheses per layer are kept (Fig. 2) and updated
  * with a Kalman filter.  The paper prints no equation for any of this; the
- * readings taken are listed in DESIGN.md ("Readings", R1..R30).
+ * readings taken are listed in DESIGN.md ("Readings", R1..R34).
  *
  * Conventions: cm, Tesla, GeV/c.  Sector frame s is rotated by (s + 1/2) * 2pi/n_sectors about
  * the beam axis; the state at local x is (y, z, sin(phi), tan(lambda), q/pT); curvature
@@ -85,6 +85,17 @@ typedef struct trd_config {
     double tan_tilt;                 /* tan of the pad tilt (2 degrees) */
     double x_ref;                    /* trd_refit: local x of the reference plane (247: the TPC outer wall of the configs) */
     double refit_var[5];             /* trd_refit: variances the covariance is reset to (y, z, sin(phi), tan(lambda), q/pT) */
+    /* Material ("taking into account ... energy loss"; R32-R34): one thin slab in front of every
+     * layer plane, crossed after the propagation to the plane and before the road (trd_refit crosses it inward after
+     * the update).  With path = sqrt((1 + tan(lambda)^2) / (1 - sin(phi)^2)), p = sqrt(1 + tan(lambda)^2) / |q/pT|,
+     * E^2 = p^2 + mass^2: scattering width theta0 = 0.0136 / (beta p) sqrt(x_over_x0 path) added to the covariance of
+     * (sin(phi), tan(lambda), q/pT); mean loss dE = eloss path / beta^2 taken from E (q/pT rescaled, direction kept), its
+     * fluctuation eloss_fluct dE added to the q/pT variance.  A particle with E - dE <= mass stops (the hypothesis
+     * only skips from then on).  x_over_x0 = eloss = 0: no material (the configs). */
+    double x_over_x0;                /* radiation lengths per layer at normal incidence, >= 0 */
+    double eloss;                    /* mean energy loss per layer [GeV] at normal incidence and beta = 1, >= 0 */
+    double eloss_fluct;              /* relative width of the energy-loss fluctuation, >= 0 */
+    double mass;                     /* mass hypothesis [GeV], >= 0 (0.13957 for pions) */
 } trd_config;
 
 /* Input tracks of one batch: device pointers, each of length n_tracks. */

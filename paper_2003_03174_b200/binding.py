@@ -38,7 +38,8 @@ class TrdConfig(C.Structure):
                 ("track_binning", C.c_int32), ("res_model", C.c_int32),
                 ("sy_c0", C.c_double), ("sy_c2", C.c_double), ("sd_c0", C.c_double), ("sd_c2", C.c_double),
                 ("sin_lorentz", C.c_double), ("tan_tilt", C.c_double), ("x_ref", C.c_double),
-                ("refit_var", C.c_double * 5)]
+                ("refit_var", C.c_double * 5),
+                ("x_over_x0", C.c_double), ("eloss", C.c_double), ("eloss_fluct", C.c_double), ("mass", C.c_double)]
 
 REFIT_VAR = (1.0, 25.0, 2.5e-3, 2.5e-3, 0.25)     # default reset variances of trd_refit (R31)
 
@@ -133,6 +134,9 @@ def make_config(cfg: dict) -> TrdConfig:
     c.x_ref = float(cfg.get("x_ref", 247.0))
     for i, v in enumerate(cfg.get("refit_var", REFIT_VAR)):
         c.refit_var[i] = float(v)
+    for k in ("x_over_x0", "eloss", "eloss_fluct"):
+        setattr(c, k, float(cfg.get(k, 0.0)))
+    c.mass = float(cfg.get("mass", 0.13957))
     return c
 
 

@@ -66,6 +66,12 @@ bool derive_params(const trd_config& c, trd::MatchParams& mp) {
     mp.tan_half = (float)tan(half);
     mp.x_ref = (float)c.x_ref;
     for (int k = 0; k < 5; ++k) mp.refit_var[k] = (float)c.refit_var[k];
+    mp.material = (c.x_over_x0 > 0.0 || c.eloss > 0.0) ? 1 : 0;
+    mp.ms_k = (float)(0.0136 * 0.0136 * c.x_over_x0);
+    mp.eloss = (float)c.eloss;
+    mp.eloss_fluct = (float)c.eloss_fluct;
+    mp.mass = (float)c.mass;
+    mp.mass2 = (float)(c.mass * c.mass);
     return true;
 }
 
@@ -93,6 +99,9 @@ const char* check_config(const trd_config& c) {
         if (!(c.sy_c0 > 0.0) || !(c.sd_c0 > 0.0) || !(c.sy_c2 >= 0.0) || !(c.sd_c2 >= 0.0)) return "resolution coefficients out of range";
         if (!(fabs(c.sin_lorentz) < 1.0) || !(fabs(c.tan_tilt) < 1.0)) return "sin_lorentz / tan_tilt out of range";
     }
+    if (!(c.x_over_x0 >= 0.0) || !(c.eloss >= 0.0) || !(c.eloss_fluct >= 0.0) || !(c.mass >= 0.0) || !isfinite(c.x_over_x0) ||
+        !isfinite(c.eloss) || !isfinite(c.eloss_fluct) || !isfinite(c.mass))
+        return "x_over_x0, eloss, eloss_fluct and mass must be finite and >= 0";
     return nullptr;
 }
 

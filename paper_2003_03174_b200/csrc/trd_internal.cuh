@@ -55,6 +55,10 @@ struct MatchParams {
     // trd_refit
     float tan_half;                  // tan(pi / n_sectors): sector edge in y = x * tan_half
     float x_ref, refit_var[5];
+    // material in front of every layer (R32-R34)
+    int material;                    // 0: none
+    float ms_k;                      // 0.0136^2 * x/X0
+    float eloss, eloss_fluct, mass, mass2;
 };
 
 struct Buffer {
