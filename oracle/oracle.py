@@ -35,6 +35,7 @@ class OrcConfig(C.Structure):
         ("sin_lorentz", C.c_double), ("tan_tilt", C.c_double), ("res_model", C.c_int32), ("pad_", C.c_int32),
         ("x_ref", C.c_double), ("refit_var", C.c_double * 5),
         ("x_over_x0", C.c_double), ("eloss", C.c_double), ("eloss_fluct", C.c_double), ("mass", C.c_double),
+        ("bz_r2", C.c_double), ("bz_z2", C.c_double),
     ]
 
 
@@ -78,6 +79,8 @@ def make_config(cfg: dict) -> OrcConfig:
     for k in ("x_over_x0", "eloss", "eloss_fluct"):
         setattr(c, k, float(cfg.get(k, 0.0)))
     c.mass = float(cfg.get("mass", PION_MASS))
+    # field inhomogeneity Bz(r, z) = bz (1 + bz_r2 r^2 + bz_z2 z^2) [R35]; absent = uniform
+    c.bz_r2 = float(cfg.get("bz_r2", 0.0)); c.bz_z2 = float(cfg.get("bz_z2", 0.0))
     return c
 
 

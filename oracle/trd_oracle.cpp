@@ -59,6 +59,9 @@ struct Config {
     // thickness in radiation lengths and mean energy loss [GeV] at normal incidence and beta = 1, relative width of
     // the energy-loss fluctuation, particle mass [GeV].  All zero = no material (the configs).
     double x_over_x0, eloss, eloss_fluct, mass;
+    // field inhomogeneity ("taking into account inhomogenities of the magnetic field") [R35]:
+    // Bz(r, z) = bz_tesla (1 + bz_r2 r^2 + bz_z2 z^2), r^2 = x^2 + y^2 [cm^2].  Both zero = uniform field (the configs).
+    double bz_r2, bz_z2;
 };
 
 struct Hyp {
@@ -85,7 +88,10 @@ struct Counters {
     int64_t n_prop = 0, n_rot = 0, n_road = 0, n_cand = 0, n_upd = 0, n_scanned = 0;
 };
 
-inline double curvature_factor(const Config& cfg) { return -0.00299792458 * cfg.bz_tesla; }
+// kappa = b q/pT; b from the field at the point (x, y, z) of the current sector frame (r^2 = x^2 + y^2 in any frame) [R35]
+inline double curvature_factor(const Config& cfg, double x, double y, double z) {
+    return -0.00299792458 * cfg.bz_tesla * (1.0 + cfg.bz_r2 * (x * x + y * y) + cfg.bz_z2 * z * z);
+}
 
 inline void note(double* margin, double value, double threshold) {
     // relative distance of a quantity from the threshold it is compared with
@@ -103,15 +109,18 @@ inline double q_of(double w) {
     return (std::asin(w) - w) / (w * w);
 }
 
-// ---- propagation x0 -> x1 inside one sector frame, uniform Bz, no material ---------------
+// ---- propagation x0 -> x1 inside one sector frame: one helix step in the field at its middle ---------------
 // PAPER.md:52 ("extrapolated to the first TRD layer"); formulas SURVEY.md 8(c).3.
 // Returns false (state untouched) if |sin(phi)| would reach max_snp [R14].  F, if given,
 // receives the 5x5 Jacobian d(y',z',s',t',c')/d(y,z,s,t,c).
 bool propagate_state(const Config& cfg, const double p[5], double x0, double x1, double out[5],
                      double F[5][5], double* margin) {
-    const double b = curvature_factor(cfg);
     const double dx = x1 - x0;
     const double y = p[0], z = p[1], s = p[2], t = p[3], c = p[4];
+    if (std::fabs(s) >= 1.0) return false;
+    // one helix step with the field taken at the middle of the straight line from the start point [R35]
+    const double r0 = std::sqrt(1.0 - s * s);
+    const double b = curvature_factor(cfg, x0 + 0.5 * dx, y + 0.5 * dx * s / r0, z + 0.5 * dx * t / r0);
     const double kappa = b * c;
     const double u = kappa * dx;
     const double f1 = s, f2 = s + u;
@@ -191,7 +200,7 @@ bool rotate_state(const Config& cfg, const double p[5], double x, double beta, d
     out[3] = p[3];
     out[4] = p[4];
     if (J) {
-        const double kappa = curvature_factor(cfg) * p[4];
+        const double kappa = curvature_factor(cfg, x, y, p[1]) * p[4];
         for (int i = 0; i < 5; ++i)
             for (int j = 0; j < 5; ++j) J[i][j] = (i == j) ? 1.0 : 0.0;
         J[0][0] = r / r2;

@@ -69,6 +69,11 @@ ELOSS = 1.5e-3                       # GeV per layer at normal incidence and bet
 ELOSS_FLUCT = 0.3                    # relative width of the energy-loss fluctuation
 HIGHLAND = 0.0136                    # GeV: theta0 = HIGHLAND / (beta p) sqrt(x/X0)
 
+# Field inhomogeneity of PAPER.md:64 (the ALICE field map is not available: synthetic, R35):
+# Bz(r, z) = Bz (1 + BZ_R2 r^2 + BZ_Z2 z^2), r, z in cm
+BZ_R2 = -1.5e-7                      # -2 % at r = 364 cm
+BZ_Z2 = -1.0e-7                      # -1.2 % at |z| = 350 cm
+
 
 @dataclasses.dataclass(frozen=True)
 class WorkloadSpec:
@@ -92,6 +97,8 @@ class WorkloadSpec:
     x_over_x0: float = 0.0            # > 0: a slab of that many radiation lengths in front of every layer:
     eloss: float = 0.0                # the true particle is scattered there and loses eloss * path / beta^2 GeV
     eloss_fluct: float = 0.0          # (Gaussian fluctuation of that relative width)
+    bz_r2: float = 0.0                # != 0: the true particle moves in Bz (1 + bz_r2 r^2 + bz_z2 z^2), integrated numerically
+    bz_z2: float = 0.0
     n_interactions: int = 0           # > 1: time-frame association: tracks i*n_ia//n_tracks form one
                                       # collision, their tracklets inherit its id, noise tracklets get a random one
 
@@ -133,6 +140,8 @@ def matcher_config(spec: WorkloadSpec) -> dict:
                      sin_lorentz=sin_lorentz(spec.bz), tan_tilt=math.tan(math.radians(TILT_DEG)))
     if spec.x_over_x0 > 0.0 or spec.eloss > 0.0:
         extra.update(x_over_x0=spec.x_over_x0, eloss=spec.eloss, eloss_fluct=spec.eloss_fluct, mass=PION_MASS)
+    if spec.bz_r2 != 0.0 or spec.bz_z2 != 0.0:
+        extra.update(bz_r2=spec.bz_r2, bz_z2=spec.bz_z2)
     return dict(extra,
         n_sectors=N_SECTORS, n_stacks=N_STACKS, n_layers=N_LAYERS,
         layer_x=list(LAYER_X), z_max=Z_MAX, pad_length=PAD_LENGTH, bz_tesla=spec.bz,
@@ -265,6 +274,70 @@ def _cross_with_sector_search(gx, gy, gz, psi, kappa, tanl, x_plane):
     return out["sec"], out["y"], out["z"], out["s"], out["ok"]
 
 
+def _rk4_path(spec, kfac, gx, gy, gz, psi, qpt, tanl, path, n_sub):
+    """Equations of motion in the field Bz(r, z) = Bz (1 + bz_r2 r^2 + bz_z2 z^2), independent variable the xy path
+    length u:  dX/du = cos(psi), dY/du = sin(psi), dZ/du = tan(lambda), dpsi/du = kfac q/pT (1 + bz_r2 (X^2 + Y^2) +
+    bz_z2 Z^2).  Classical Runge-Kutta over `path` (array, per particle) in n_sub equal steps."""
+    def rhs(X, Y, Z, P):
+        return np.cos(P), np.sin(P), tanl, kfac * qpt * (1.0 + spec.bz_r2 * (X * X + Y * Y) + spec.bz_z2 * Z * Z)
+    h = path / n_sub
+    X, Y, Z, P = gx.copy(), gy.copy(), gz.copy(), psi.copy()
+    for _ in range(n_sub):
+        a = rhs(X, Y, Z, P)
+        b = rhs(X + 0.5 * h * a[0], Y + 0.5 * h * a[1], Z + 0.5 * h * a[2], P + 0.5 * h * a[3])
+        c = rhs(X + 0.5 * h * b[0], Y + 0.5 * h * b[1], Z + 0.5 * h * b[2], P + 0.5 * h * b[3])
+        d = rhs(X + h * c[0], Y + h * c[1], Z + h * c[2], P + h * c[3])
+        X = X + h / 6.0 * (a[0] + 2.0 * b[0] + 2.0 * c[0] + d[0])
+        Y = Y + h / 6.0 * (a[1] + 2.0 * b[1] + 2.0 * c[1] + d[1])
+        Z = Z + h / 6.0 * (a[2] + 2.0 * b[2] + 2.0 * c[2] + d[2])
+        P = P + h / 6.0 * (a[3] + 2.0 * b[3] + 2.0 * c[3] + d[3])
+    return X, Y, Z, P
+
+
+def _cross_rk4(spec, kfac, gx, gy, gz, psi, qpt, tanl, x_plane, sec, n_sub):
+    """Like _cross_from, in the inhomogeneous field: the path length to the plane is found by Newton's method
+    (start: the uniform-field helix), each trial integrated from the start point with _rk4_path."""
+    alpha = (sec + 0.5) * SECTOR_WIDTH
+    ca, sa = np.cos(alpha), np.sin(alpha)
+    x0 = gx * ca + gy * sa
+    ploc = np.mod(psi - alpha + np.pi, 2.0 * np.pi) - np.pi
+    kappa = kfac * qpt
+    s0 = np.sin(ploc)
+    s1 = s0 + kappa * (x_plane - x0)
+    ok = (np.abs(s1) < 1.0) & (np.cos(ploc) > 0.0)
+    s1c = np.where(ok, s1, s0)
+    straight = np.abs(kappa) < 1e-12
+    path = np.where(straight, (x_plane - x0) / np.where(ok, np.cos(ploc), 1.0),
+                    (np.arcsin(s1c) - np.arcsin(np.clip(s0, -1, 1))) / np.where(straight, 1.0, kappa))
+    path = np.where(ok, path, 0.0)
+    for _ in range(4):
+        X, Y, Z, P = _rk4_path(spec, kfac, gx, gy, gz, psi, qpt, tanl, path, n_sub)
+        cl = np.cos(P - alpha)
+        ok &= cl > 0.05
+        path = path + np.where(ok, (x_plane - (X * ca + Y * sa)) / np.where(ok, cl, 1.0), 0.0)
+    X, Y, Z, P = _rk4_path(spec, kfac, gx, gy, gz, psi, qpt, tanl, path, n_sub)
+    ok &= np.abs(X * ca + Y * sa - x_plane) < 1e-9
+    return -X * sa + Y * ca, Z, np.sin(P - alpha), ok
+
+
+def _cross_rk4_search(spec, kfac, gx, gy, gz, psi, qpt, tanl, x_plane, n_sub):
+    """_cross_rk4 in the sector whose |y| <= x_plane tan(10 deg): the sector found with the uniform-field helix
+    first, its neighbour on the side of y where that fails."""
+    sec, _, _, _, okh = _cross_with_sector_search(gx, gy, gz, psi, kfac * qpt, tanl, x_plane)
+    y, z, s1, ok = _cross_rk4(spec, kfac, gx, gy, gz, psi, qpt, tanl, x_plane, sec, n_sub)
+    edge = x_plane * TAN_HALF_SECTOR
+    with np.errstate(invalid="ignore"):
+        out = okh & ok & (np.abs(y) > edge)
+    if out.any():
+        i = np.nonzero(out)[0]
+        sec2 = np.mod(sec[i] + np.where(y[i] > 0, 1, -1), N_SECTORS)
+        y2, z2, s2, ok2 = _cross_rk4(spec, kfac, gx[i], gy[i], gz[i], psi[i], qpt[i], tanl[i], x_plane, sec2, n_sub)
+        sec, y, z, s1, ok = sec.copy(), y.copy(), z.copy(), s1.copy(), ok.copy()
+        sec[i], y[i], z[i], s1[i] = sec2, y2, z2, s2
+        ok[i] = ok2 & (np.abs(y2) <= edge)
+    return sec, y, z, s1, okh & ok
+
+
 def chamber_offsets(spec: "WorkloadSpec") -> np.ndarray:
     """Radial offset of every chamber from its nominal layer plane (float32 cm), own seeded stream."""
     n_ch = N_SECTORS * N_STACKS * N_LAYERS
@@ -302,6 +375,14 @@ def generate(spec: WorkloadSpec) -> dict:
     n = spec.n_tracks
     kfac = KAPPA_PER_TESLA * spec.bz
 
+    field = spec.bz_r2 != 0.0 or spec.bz_z2 != 0.0
+
+    def from_origin(phi0_, qpt_, tanl_, x_plane):
+        if not field:
+            return _truth_at_plane(phi0_, kfac * qpt_, tanl_, x_plane)
+        zero = np.zeros_like(phi0_)
+        return _cross_rk4_search(spec, kfac, zero, zero, zero, phi0_, qpt_, tanl_, x_plane, 32)
+
     # 1. particles, redrawn in blocks of n until n of them reach x = 247 and layer 0 (draw order:
     #    q, pT, eta, phi0 per block)
     keep = {k: [] for k in ("q", "pt", "tanl", "phi0")}
@@ -309,8 +390,8 @@ def generate(spec: WorkloadSpec) -> dict:
     while have < n:
         q, pt, tanl, phi0 = _draw_particles(rng, spec, max(n, 64))
         kappa = kfac * q / pt
-        _, _, _, s_seed, ok_seed = _truth_at_plane(phi0, kappa, tanl, X_SEED)
-        _, _, _, s_l0, ok_l0 = _truth_at_plane(phi0, kappa, tanl, LAYER_X[0])
+        _, _, _, s_seed, ok_seed = from_origin(phi0, q / pt, tanl, X_SEED)
+        _, _, _, s_l0, ok_l0 = from_origin(phi0, q / pt, tanl, LAYER_X[0])
         good = ok_seed & ok_l0 & (np.abs(s_seed) < MAX_SNP) & (np.abs(s_l0) < MAX_SNP)
         for k, v in (("q", q), ("pt", pt), ("tanl", tanl), ("phi0", phi0)):
             keep[k].append(v[good])
@@ -320,7 +401,7 @@ def generate(spec: WorkloadSpec) -> dict:
     kappa = kfac * qpt
 
     # 2. seed state at x = 247 (+ smearing, draw order: 5 normals per track as one (n, 5) block)
-    sec, y, z, s, ok = _truth_at_plane(phi0, kappa, tanl, X_SEED)
+    sec, y, z, s, ok = from_origin(phi0, qpt, tanl, X_SEED)
     assert ok.all()
     truth_par = np.stack([y, z, s, tanl, qpt])
     sig = np.stack([np.full(n, SIGMA_SEED[0]), np.full(n, SIGMA_SEED[1]), np.full(n, SIGMA_SEED[2]),
@@ -336,18 +417,25 @@ def generate(spec: WorkloadSpec) -> dict:
     truth_last = np.full((n, 4), np.nan)
     ch_dx = chamber_offsets(spec)
     material = spec.x_over_x0 > 0.0 or spec.eloss > 0.0
-    if material:
+    stepped = material or field
+    if stepped:
         # stepped truth: global point, azimuth, tan(lambda), q/pT after the last slab crossed (the origin at first)
         gx, gy, gz = np.zeros(n), np.zeros(n), np.zeros(n)
         psi, tl_now, qpt_now, going = phi0.copy(), tanl.copy(), qpt.copy(), np.ones(n, bool)
         truth_last_par = np.full((5, n), np.nan)
     for lay, xl in enumerate(LAYER_X):
-        if material:
+        if stepped:
             # crossing of the nominal plane, then the slab: two scattering angles and the energy loss
-            # (draw order per layer: k1, k2, ke, then the draws of the plain generator)
-            secl, yl, zl, sl, okl = _cross_with_sector_search(gx, gy, gz, psi, kfac * qpt_now, tl_now, xl)
+            # (draw order per layer: k1, k2, ke, then the draws of the plain generator; no slab draws without material)
+            if field:
+                secl, yl, zl, sl, okl = _cross_rk4_search(spec, kfac, gx, gy, gz, psi, qpt_now, tl_now, xl, 32 if lay == 0 else 8)
+            else:
+                secl, yl, zl, sl, okl = _cross_with_sector_search(gx, gy, gz, psi, kfac * qpt_now, tl_now, xl)
             okl &= going
-            k1, k2, ke = rng.standard_normal(n), rng.standard_normal(n), rng.standard_normal(n)
+            if material:
+                k1, k2, ke = rng.standard_normal(n), rng.standard_normal(n), rng.standard_normal(n)
+            else:
+                k1 = k2 = ke = 0.0
             with np.errstate(invalid="ignore"):
                 sc = np.where(okl, sl, 0.0)
                 path = np.sqrt((1.0 + tl_now ** 2) / (1.0 - sc * sc))
@@ -379,7 +467,7 @@ def generate(spec: WorkloadSpec) -> dict:
             present = okl & (np.abs(zl) < Z_MAX) & (np.abs(sl) < MAX_SNP) & (u < spec.efficiency)
         if lay == N_LAYERS - 1:
             truth_last[okl] = np.stack([yl, zl, sl, secl.astype(float)], axis=1)[okl]
-            if material:
+            if stepped:
                 truth_last_par[:, okl] = np.stack([yl, zl, sl, tl_now, qpt_now])[:, okl]
         idx = np.nonzero(present)[0]
         chamber_l = secl[idx] * (N_STACKS * N_LAYERS) + stack_of_z(pad_row_centre(zl[idx])) * N_LAYERS + lay
@@ -387,7 +475,9 @@ def generate(spec: WorkloadSpec) -> dict:
             # the chamber sits at x_l + dx: the tracklet is measured where the particle crosses THAT plane
             yl, zl, sl = yl.copy(), zl.copy(), sl.copy()
             xd = xl + ch_dx[chamber_l].astype(np.float64)
-            if material:
+            if field:
+                yd, zd, sd, okd = _cross_rk4(spec, kfac, gx[idx], gy[idx], gz[idx], psi[idx], qpt_now[idx], tl_now[idx], xd, secl[idx], 2)
+            elif material:
                 yd, zd, sd, okd = _cross_from(gx[idx], gy[idx], gz[idx], psi[idx], kfac * qpt_now[idx], tl_now[idx], xd, secl[idx])
             else:
                 yd, zd, sd, okd = _truth_in_sector(phi0[idx], kappa[idx], tanl[idx], xd, secl[idx])
@@ -448,7 +538,7 @@ def generate(spec: WorkloadSpec) -> dict:
 
     if spec.chamber_dx_sigma > 0.0:
         assoc["chamber_dx"] = ch_dx
-    if material:
+    if stepped:
         assoc["truth_last_par"] = truth_last_par
     return dict(
         assoc, spec=spec,
