@@ -377,6 +377,8 @@ def main():
                     help="> 0: chambers displaced radially by N(0, this) cm, two-stage propagation (SURVEY.md 8(f) NEXT#3)")
     ap.add_argument("--material", action="store_true",
                     help="a slab of material in front of every layer: multiple scattering and energy loss (SURVEY.md 8(f) NEXT#3)")
+    ap.add_argument("--field", action="store_true",
+                    help="inhomogeneous field Bz (1 + bz_r2 r^2 + bz_z2 z^2), true particles integrated numerically (SURVEY.md 8(f) NEXT#3)")
     ap.add_argument("--res-model", type=int, default=0, choices=[0, 1],
                     help="1: inputs and matcher with the sin(phi)-dependent resolutions and pad tilt (SURVEY.md 8(f) NEXT#1)")
     args = ap.parse_args()
@@ -393,6 +395,8 @@ def main():
         spec = dataclasses.replace(spec, chamber_dx_sigma=args.chamber_dx, name=spec.name + "_dx")
     if args.material:
         spec = dataclasses.replace(spec, x_over_x0=W.X_OVER_X0, eloss=W.ELOSS, eloss_fluct=W.ELOSS_FLUCT, name=spec.name + "_mat")
+    if args.field:
+        spec = dataclasses.replace(spec, bz_r2=W.BZ_R2, bz_z2=W.BZ_Z2, name=spec.name + "_field")
     cfg = W.matcher_config(spec)
     if args.ybin_width > 0.0:
         cfg["ybin_width"] = args.ybin_width

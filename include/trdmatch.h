@@ -7,7 +7,7 @@
  * inclination is more than n_sigma_angle sigma off the track inclination are excluded
  * (PAPER.md:60), the best n_hyp hypotheses per layer are kept (Fig. 2) and updated
  * with a Kalman filter.  The paper prints no equation for any of this; the
- * readings taken are listed in DESIGN.md ("Readings", R1..R34).
+ * readings taken are listed in DESIGN.md ("Readings", R1..R35).
  *
  * Conventions: cm, Tesla, GeV/c.  Sector frame s is rotated by (s + 1/2) * 2pi/n_sectors about
  * the beam axis; the state at local x is (y, z, sin(phi), tan(lambda), q/pT); curvature
@@ -96,6 +96,12 @@ typedef struct trd_config {
     double eloss;                    /* mean energy loss per layer [GeV] at normal incidence and beta = 1, >= 0 */
     double eloss_fluct;              /* relative width of the energy-loss fluctuation, >= 0 */
     double mass;                     /* mass hypothesis [GeV], >= 0 (0.13957 for pions) */
+    /* Field inhomogeneity ("taking into account inhomogenities of the magnetic field"; R35):
+     * Bz(r, z) = bz_tesla (1 + bz_r2 r^2 + bz_z2 z^2), r^2 = x^2 + y^2, in cm.  Every propagation stays one helix step,
+     * with the field at the middle of the straight line from its start point.  Both zero: uniform field (the configs).
+     * The factor must stay positive inside the detector: 1 + bz_r2 R^2 + bz_z2 z_max^2 > 0.5 with R the last layer's
+     * outer corner. */
+    double bz_r2, bz_z2;             /* [1/cm^2] */
 } trd_config;
 
 /* Input tracks of one batch: device pointers, each of length n_tracks. */

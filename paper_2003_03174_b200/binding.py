@@ -39,7 +39,8 @@ class TrdConfig(C.Structure):
                 ("sy_c0", C.c_double), ("sy_c2", C.c_double), ("sd_c0", C.c_double), ("sd_c2", C.c_double),
                 ("sin_lorentz", C.c_double), ("tan_tilt", C.c_double), ("x_ref", C.c_double),
                 ("refit_var", C.c_double * 5),
-                ("x_over_x0", C.c_double), ("eloss", C.c_double), ("eloss_fluct", C.c_double), ("mass", C.c_double)]
+                ("x_over_x0", C.c_double), ("eloss", C.c_double), ("eloss_fluct", C.c_double), ("mass", C.c_double),
+                ("bz_r2", C.c_double), ("bz_z2", C.c_double)]
 
 REFIT_VAR = (1.0, 25.0, 2.5e-3, 2.5e-3, 0.25)     # default reset variances of trd_refit (R31)
 
@@ -137,6 +138,7 @@ def make_config(cfg: dict) -> TrdConfig:
     for k in ("x_over_x0", "eloss", "eloss_fluct"):
         setattr(c, k, float(cfg.get(k, 0.0)))
     c.mass = float(cfg.get("mass", 0.13957))
+    c.bz_r2 = float(cfg.get("bz_r2", 0.0)); c.bz_z2 = float(cfg.get("bz_z2", 0.0))
     return c
 
 

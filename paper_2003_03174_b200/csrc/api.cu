@@ -72,6 +72,9 @@ bool derive_params(const trd_config& c, trd::MatchParams& mp) {
     mp.eloss_fluct = (float)c.eloss_fluct;
     mp.mass = (float)c.mass;
     mp.mass2 = (float)(c.mass * c.mass);
+    mp.field = (c.bz_r2 != 0.0 || c.bz_z2 != 0.0) ? 1 : 0;
+    mp.bz_r2 = (float)c.bz_r2;
+    mp.bz_z2 = (float)c.bz_z2;
     return true;
 }
 
@@ -102,6 +105,13 @@ const char* check_config(const trd_config& c) {
     if (!(c.x_over_x0 >= 0.0) || !(c.eloss >= 0.0) || !(c.eloss_fluct >= 0.0) || !(c.mass >= 0.0) || !isfinite(c.x_over_x0) ||
         !isfinite(c.eloss) || !isfinite(c.eloss_fluct) || !isfinite(c.mass))
         return "x_over_x0, eloss, eloss_fluct and mass must be finite and >= 0";
+    if (!isfinite(c.bz_r2) || !isfinite(c.bz_z2)) return "bz_r2 / bz_z2 not finite";
+    {   // the field factor must stay well above zero inside the detector
+        const double xl = c.layer_x[c.n_layers - 1], half = M_PI / c.n_sectors;
+        const double r2 = xl * xl * (1.0 + tan(half) * tan(half));
+        const double lo = 1.0 + (c.bz_r2 < 0.0 ? c.bz_r2 * r2 : 0.0) + (c.bz_z2 < 0.0 ? c.bz_z2 * c.z_max * c.z_max : 0.0);
+        if (!(lo > 0.5)) return "bz_r2 / bz_z2 take more than half of the field away inside the detector";
+    }
     return nullptr;
 }
 

@@ -59,6 +59,9 @@ struct MatchParams {
     int material;                    // 0: none
     float ms_k;                      // 0.0136^2 * x/X0
     float eloss, eloss_fluct, mass, mass2;
+    // field inhomogeneity Bz (1 + bz_r2 r^2 + bz_z2 z^2) (R35)
+    int field;                       // 0: uniform
+    float bz_r2, bz_z2;
 };
 
 struct Buffer {
