@@ -381,7 +381,7 @@ def generate(spec: WorkloadSpec) -> dict:
         if not field:
             return _truth_at_plane(phi0_, kfac * qpt_, tanl_, x_plane)
         zero = np.zeros_like(phi0_)
-        return _cross_rk4_search(spec, kfac, zero, zero, zero, phi0_, qpt_, tanl_, x_plane, 32)
+        return _cross_rk4_search(spec, kfac, zero, zero, zero, phi0_, qpt_, tanl_, x_plane, 64)
 
     # 1. particles, redrawn in blocks of n until n of them reach x = 247 and layer 0 (draw order:
     #    q, pT, eta, phi0 per block)
@@ -428,7 +428,7 @@ def generate(spec: WorkloadSpec) -> dict:
             # crossing of the nominal plane, then the slab: two scattering angles and the energy loss
             # (draw order per layer: k1, k2, ke, then the draws of the plain generator; no slab draws without material)
             if field:
-                secl, yl, zl, sl, okl = _cross_rk4_search(spec, kfac, gx, gy, gz, psi, qpt_now, tl_now, xl, 32 if lay == 0 else 8)
+                secl, yl, zl, sl, okl = _cross_rk4_search(spec, kfac, gx, gy, gz, psi, qpt_now, tl_now, xl, 64 if lay == 0 else 8)
             else:
                 secl, yl, zl, sl, okl = _cross_with_sector_search(gx, gy, gz, psi, kfac * qpt_now, tl_now, xl)
             okl &= going
