@@ -3,8 +3,10 @@
 // Tracks arrive in arbitrary order, so neighbouring sub-warps of the match kernel would touch
 // unrelated bins of the tracklet index and re-read it from HBM many times.  For large batches
 // trd_match therefore (1) packs every track into one 96-byte record and computes a locality key
-// (sector, z row, coarse y of the straight-line prediction at the middle TRD layer), (2) radix-sorts
-// the keys (index.cu), (3) runs the match kernel over the sorted permutation, gathering whole
+// (sector, z row, coarse y of the straight-line prediction at the middle TRD layer), (2) orders the
+// tracks by key -- a counting sort (histogram by atomics in the pack kernel, one-block scan, placement
+// by atomics; the order inside a key is arbitrary and irrelevant) when the key has at most 16 bits,
+// else the radix sort of index.cu --, (3) runs the match kernel over the permutation, gathering whole
 // records and scattering whole 128-byte result records, (4) unpacks the results to the caller's
 // SoA arrays.  The key only decides the processing order; no result depends on it.
 #include "trd_internal.cuh"
@@ -19,7 +21,7 @@ constexpr int kYBits = 4;                      // 16 coarse y bins per (sector, 
 // SoA -> records through shared memory so that both sides are coalesced
 __global__ void __launch_bounds__(kThreads) pack_kernel(const trd_tracks_in in, int64_t n, float* __restrict__ rec,
                                                         uint32_t* __restrict__ key, IndexGeom g, float x_mid, float edge_mid,
-                                                        int nz) {
+                                                        int nz, uint32_t* __restrict__ hist) {
     __shared__ float sm[kThreads][kRecIn + 1];
     const int64_t base = (int64_t)blockIdx.x * kThreads;
     const int64_t i = base + threadIdx.x;
@@ -49,12 +51,15 @@ __global__ void __launch_bounds__(kThreads) pack_kernel(const trd_tracks_in in, 
         float fy = floorf((yp + edge_mid) / (2.0f * edge_mid) * (float)(1 << kYBits));
         fy = fminf(fmaxf(fy, 0.0f), (float)((1 << kYBits) - 1));
         const int zr = isfinite(zp) ? zrow_of(g, zp) : 0;
+        uint32_t kk;
         if (g.n_ia > 1) {      // with association the interaction leads, as in the tracklet index
             const int a = min(max(ia, 0), g.n_ia - 1);
-            key[i] = ((uint32_t)a * (uint32_t)g.n_sectors + (uint32_t)sec) * (uint32_t)nz + (uint32_t)zr;
+            kk = ((uint32_t)a * (uint32_t)g.n_sectors + (uint32_t)sec) * (uint32_t)nz + (uint32_t)zr;
         } else {
-            key[i] = (((uint32_t)sec * (uint32_t)nz + (uint32_t)zr) << kYBits) + (uint32_t)(isfinite(fy) ? (int)fy : 0);
+            kk = (((uint32_t)sec * (uint32_t)nz + (uint32_t)zr) << kYBits) + (uint32_t)(isfinite(fy) ? (int)fy : 0);
         }
+        key[i] = kk;
+        if (hist) atomicAdd(hist + kk, 1u);
     }
     __syncthreads();
     const int64_t n_here = min((int64_t)kThreads, n - base);
@@ -96,22 +101,98 @@ __global__ void __launch_bounds__(kThreads) unpack_kernel(const float* __restric
     if (out.n_cand_evals) out.n_cand_evals[i] = __float_as_int(r[30]);
 }
 
+// counting sort, step 2: exclusive scan of the key histogram in place (one block)
+constexpr int kScanThreads = 1024;
+constexpr int kScanMax = (1 << kCountingBits) / kScanThreads;      // keys per thread at most (64)
+__global__ void __launch_bounds__(kScanThreads) scan_hist(uint32_t* __restrict__ hist, int per4) {
+    // thread t owns the 4 * per4 consecutive keys from t * 4 * per4 (n_keys = 1024 * 4 * per4, a power of two >= 4096);
+    // 16-byte loads, all issued before the first use
+    __shared__ uint32_t warp_sums[32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    uint4* mine = reinterpret_cast<uint4*>(hist) + (size_t)threadIdx.x * per4;
+    uint4 c[kScanMax / 4];
+#pragma unroll
+    for (int k = 0; k < kScanMax / 4; ++k) c[k] = (k < per4) ? mine[k] : make_uint4(0u, 0u, 0u, 0u);
+    uint32_t sum = 0;
+#pragma unroll
+    for (int k = 0; k < kScanMax / 4; ++k) sum += c[k].x + c[k].y + c[k].z + c[k].w;
+    uint32_t incl = sum;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t t = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += t;
+    }
+    if (lane == 31) warp_sums[warp] = incl;
+    __syncthreads();
+    if (warp == 0) {
+        const uint32_t w = warp_sums[lane];
+        uint32_t wi = w;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t t = __shfl_up_sync(0xffffffffu, wi, o);
+            if (lane >= o) wi += t;
+        }
+        warp_sums[lane] = wi - w;
+    }
+    __syncthreads();
+    uint32_t run = warp_sums[warp] + incl - sum;
+#pragma unroll
+    for (int k = 0; k < kScanMax / 4; ++k) {
+        if (k < per4) {
+            uint4 o;
+            o.x = run; run += c[k].x;
+            o.y = run; run += c[k].y;
+            o.z = run; run += c[k].z;
+            o.w = run; run += c[k].w;
+            mine[k] = o;
+        }
+    }
+}
+
+// counting sort, step 3: every track takes the next free place of its key
+__global__ void __launch_bounds__(256) place_tracks(const uint32_t* __restrict__ key, uint32_t* __restrict__ next,
+                                                    uint32_t* __restrict__ perm, int64_t n) {
+    const int64_t i = (int64_t)blockIdx.x * 256 + threadIdx.x;
+    if (i < n) perm[atomicAdd(next + key[i], 1u)] = (uint32_t)i;
+}
+
 }  // namespace
 
 cudaError_t pack_tracks(trd_handle* h, const trd_tracks_in& in, int64_t n, float* rec, uint32_t* key, int* key_bits,
-                        cudaStream_t stream) {
+                        uint32_t* hist, cudaStream_t stream) {
     const trd_config& c = h->cfg;
     const IndexGeom& g = h->mp.g;
     const int mid = c.n_layers / 2;
     const float x_mid = (float)c.layer_x[mid];
     const float edge_mid = (float)(c.layer_x[mid] * tan(M_PI / c.n_sectors));
     const unsigned grid = (unsigned)((n + kThreads - 1) / kThreads);
-    pack_kernel<<<grid, kThreads, 0, stream>>>(in, n, rec, key, g, x_mid, edge_mid, g.nz);
+    const int bits = track_key_bits(h);
+    if (bits > kCountingBits) hist = nullptr;
+    if (hist) {
+        cudaError_t e = cudaMemsetAsync(hist, 0, sizeof(uint32_t) << bits, stream);
+        if (e != cudaSuccess) return e;
+    }
+    pack_kernel<<<grid, kThreads, 0, stream>>>(in, n, rec, key, g, x_mid, edge_mid, g.nz, hist);
     h->launches++;
-    uint64_t n_keys = g.n_ia > 1 ? (uint64_t)g.n_ia * c.n_sectors * g.nz : ((uint64_t)c.n_sectors * g.nz) << kYBits;
+    *key_bits = bits;
+    return cudaGetLastError();
+}
+
+int track_key_bits(const trd_handle* h) {
+    const trd_config& c = h->cfg;
+    const IndexGeom& g = h->mp.g;
+    const uint64_t n_keys = g.n_ia > 1 ? (uint64_t)g.n_ia * c.n_sectors * g.nz : ((uint64_t)c.n_sectors * g.nz) << kYBits;
     int bits = 0;
     while ((1ull << bits) < n_keys) ++bits;
-    *key_bits = bits;
+    return bits < 12 ? 12 : bits;        // the one-block scan of the counting sort wants at least 4 keys per thread
+}
+
+// counting sort of the tracks by the key histogram pack_tracks filled: perm[place] = track
+cudaError_t place_tracks_by_key(trd_handle* h, const uint32_t* key, uint32_t* hist, uint32_t* perm, int key_bits, int64_t n,
+                                cudaStream_t stream) {
+    scan_hist<<<1, kScanThreads, 0, stream>>>(hist, (1 << key_bits) / (4 * kScanThreads));
+    place_tracks<<<(unsigned)((n + 255) / 256), 256, 0, stream>>>(key, hist, perm, n);
+    h->launches += 2;
     return cudaGetLastError();
 }
 

@@ -138,8 +138,12 @@ cudaError_t radix_sort_pairs(uint32_t* key0, uint32_t* key1, uint32_t* val0, uin
                              uint32_t* digit_tot, int64_t n, int n_passes, cudaStream_t stream, int* side_out,
                              int64_t* launches);
 // tracks.cu: SoA -> packed records + locality key; packed results -> SoA
+constexpr int kCountingBits = 16;     // track keys up to this many bits are counting-sorted (tracks.cu)
+int track_key_bits(const trd_handle* h);
 cudaError_t pack_tracks(trd_handle* h, const trd_tracks_in& in, int64_t n, float* rec, uint32_t* key, int* key_bits,
-                        cudaStream_t stream);
+                        uint32_t* hist, cudaStream_t stream);
+cudaError_t place_tracks_by_key(trd_handle* h, const uint32_t* key, uint32_t* hist, uint32_t* perm, int key_bits, int64_t n,
+                                cudaStream_t stream);
 cudaError_t unpack_tracks(trd_handle* h, const float* rec_out, const trd_tracks_out& out, int64_t n, cudaStream_t stream);
 
 int fail(trd_handle* h, int code, const std::string& what);
