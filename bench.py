@@ -113,6 +113,16 @@ def load_units(spec, n_batches):
     return u["batches"]
 
 
+def load_bytes(info: dict, n_tl: int) -> float:
+    """Bytes trd_load_tracklets has to move with the sort it used: the radix path reads the SoA (16),
+    writes record + key (20), per pass 4 + 8 + 8, then gathers (4 + 4 + 16 + 16); the counting path reads the SoA (16),
+    writes record + key (20), partitions (20 + 20), places (20 + 16), orders (16) and passes five times over the
+    4-byte bin table."""
+    if info["sort_kind"] == 1:
+        return n_tl * 128.0 + 20.0 * info["n_bins"]
+    return n_tl * (76.0 + 20.0 * info["n_passes"])
+
+
 def config_dict(spec, n_tl, world):
     n, batch = spec.n_tracks, spec.batch or spec.n_tracks
     nb = (n + batch - 1) // batch
@@ -326,7 +336,8 @@ def run_ours(args, spec, cfg):
                 roofline_ms_per_launch=1e3 * max(t_alu, t_hbm), hbm_view_gbs=bytes_alg / (match_avg_ms * 1e-3) / 1e9,
                 peak_source=f"HBM {peaks['source']} (MEASURED_PEAKS.json); FP32 = {props.multi_processor_count} SMs x 128 x 2 x "
                             f"{peaks['sm_max_mhz']:.0f} MHz", units=units_src,
-                load_tracklets_ms=load_ms, load_algorithmic_gbs=n_tl * (52 + 20 * info["n_passes"]) / (load_ms * 1e-3) / 1e9)
+                load_tracklets_ms=load_ms, load_algorithmic_gbs=load_bytes(info, n_tl) / (load_ms * 1e-3) / 1e9,
+                load_io_gbs=n_tl * 32 / (load_ms * 1e-3) / 1e9)
     prof = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(prof):
         with open(prof) as f:
@@ -338,7 +349,9 @@ def run_ours(args, spec, cfg):
                 config=config_dict(spec, n_tl, world),
                 cand_evals_per_s=world * n_evals / (ms_per_step * 1e-3), n_cand_evals=n_evals,
                 frac_tracks_ge2_tracklets=n_ge2 / n, index=dict(n_ybins=info["n_ybins"], n_zrows=info["n_zrows"],
-                                                                ybin_width_cm=info["ybin_width"], radix_passes=info["n_passes"]),
+                                                                ybin_width_cm=info["ybin_width"],
+                                                                sort="counting" if info["sort_kind"] == 1 else "radix",
+                                                                radix_passes=0 if info["sort_kind"] == 1 else info["n_passes"]),
                 refit=dict(ms_per_time_frame=refit_ms, tracks_per_s=n / (refit_ms * 1e-3), frac_refitted=n_refitted / n,
                            note="trd_refit over the matched chains of the step, device-resident, timed separately"),
                 clocks=clocks, gpu_launches=int(launches),

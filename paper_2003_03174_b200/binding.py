@@ -40,7 +40,7 @@ class TrdConfig(C.Structure):
                 ("sin_lorentz", C.c_double), ("tan_tilt", C.c_double), ("x_ref", C.c_double),
                 ("refit_var", C.c_double * 5),
                 ("x_over_x0", C.c_double), ("eloss", C.c_double), ("eloss_fluct", C.c_double), ("mass", C.c_double),
-                ("bz_r2", C.c_double), ("bz_z2", C.c_double)]
+                ("bz_r2", C.c_double), ("bz_z2", C.c_double), ("index_sort", C.c_int32), ("reserved_", C.c_int32)]
 
 REFIT_VAR = (1.0, 25.0, 2.5e-3, 2.5e-3, 0.25)     # default reset variances of trd_refit (R31)
 
@@ -64,7 +64,7 @@ class TrdRefitOut(C.Structure):
 class TrdIndexInfo(C.Structure):
     _fields_ = [("n_tracklets", C.c_int64), ("n_zrows", C.c_int32), ("n_ybins", C.c_int32), ("n_bins", C.c_int64),
                 ("ybin_width", C.c_double), ("key_bits", C.c_int32), ("n_passes", C.c_int32),
-                ("n_interactions", C.c_int32), ("reserved_", C.c_int32)]
+                ("n_interactions", C.c_int32), ("sort_kind", C.c_int32)]
 
 
 class TrdError(RuntimeError):
@@ -139,6 +139,7 @@ def make_config(cfg: dict) -> TrdConfig:
         setattr(c, k, float(cfg.get(k, 0.0)))
     c.mass = float(cfg.get("mass", 0.13957))
     c.bz_r2 = float(cfg.get("bz_r2", 0.0)); c.bz_z2 = float(cfg.get("bz_z2", 0.0))
+    c.index_sort = int(cfg.get("index_sort", 0)); c.reserved_ = 0
     return c
 
 
@@ -355,6 +356,7 @@ def trd_copy_index(h, stream=None) -> dict:
     n = info["n_tracklets"]
     pos = np.empty(n, np.int32); key = np.empty(n, np.uint32); first = np.empty(info["n_bins"] + 1, np.int32)
     _check(h, lib().trd_copy_index(h, pos.ctypes.data, key.ctypes.data, first.ctypes.data, _stream(stream)))
+    info = trd_get_index_info(h)                    # sort_kind is final only now
     return dict(info, sorted_pos=pos, sorted_key=key, bin_first=first)
 
 

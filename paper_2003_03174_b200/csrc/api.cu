@@ -97,6 +97,7 @@ const char* check_config(const trd_config& c) {
     if (!(c.max_snp > 0.0) || !(c.max_snp < 1.0)) return "max_snp must be in (0, 1)";
     if (!(c.ybin_width >= 0.0)) return "ybin_width must be >= 0";
     if (c.track_binning < -1 || c.track_binning > 1) return "track_binning must be -1, 0 or 1";
+    if (c.index_sort < -1 || c.index_sort > 1) return "index_sort must be -1, 0 or 1";
     if (c.res_model != 0 && c.res_model != 1) return "res_model must be 0 or 1";
     if (c.res_model == 1) {
         if (!(c.sy_c0 > 0.0) || !(c.sd_c0 > 0.0) || !(c.sy_c2 >= 0.0) || !(c.sd_c2 >= 0.0)) return "resolution coefficients out of range";
@@ -160,6 +161,10 @@ void trd_destroy(trd_handle* h) {
     release(h->tile_hist);
     release(h->digit_tot);
     release(h->bin_first);
+    release(h->sort_flag);
+    release(h->scan_partial);
+    release(h->part_rec);
+    release(h->part_dx);
     release(h->row_ext);
     release(h->chamber_dx);
     release(h->store_dx);
@@ -276,7 +281,7 @@ int trd_get_index_info(const trd_handle* h, trd_index_info* info) {
     info->key_bits = h->key_bits;
     info->n_passes = h->n_passes;
     info->n_interactions = h->mp.g.n_ia;
-    info->reserved_ = 0;
+    info->sort_kind = h->sort_kind;
     return TRD_OK;
 }
 
@@ -286,6 +291,7 @@ int trd_copy_index(trd_handle* h, int32_t* sorted_pos, uint32_t* sorted_key, int
     cudaStream_t st = (cudaStream_t)stream;
     cudaError_t e = cudaStreamSynchronize(st);
     const size_t n = (size_t)h->n_tracklets;
+    if (e == cudaSuccess) e = trd::export_sorted_index(h, st);
     if (e == cudaSuccess && sorted_pos && n)
         e = cudaMemcpy(sorted_pos, h->val[h->sorted_side].p, n * 4, cudaMemcpyDeviceToHost);
     if (e == cudaSuccess && sorted_key && n)
@@ -300,7 +306,7 @@ const char* trd_last_error(const trd_handle* h) { return h ? h->err.c_str() : "N
 
 int64_t trd_device_bytes(const trd_handle* h) {
     if (!h) return 0;
-    size_t t = h->store.bytes + h->packed.bytes + h->tile_hist.bytes + h->digit_tot.bytes + h->bin_first.bytes + h->row_ext.bytes + h->chamber_dx.bytes + h->store_dx.bytes + h->stage_tl.bytes + h->trk_rec.bytes + h->trk_out.bytes + h->trk_hist.bytes +
+    size_t t = h->store.bytes + h->packed.bytes + h->part_rec.bytes + h->part_dx.bytes + h->scan_partial.bytes + h->tile_hist.bytes + h->digit_tot.bytes + h->bin_first.bytes + h->row_ext.bytes + h->chamber_dx.bytes + h->store_dx.bytes + h->stage_tl.bytes + h->trk_rec.bytes + h->trk_out.bytes + h->trk_hist.bytes +
                h->trk_tot.bytes;
     for (int s = 0; s < 2; ++s) t += h->key[s].bytes + h->val[s].bytes + h->trk_key[s].bytes + h->trk_val[s].bytes;
     return (int64_t)t;

@@ -6,6 +6,13 @@
 //       gather_store     sorted store: one float4 (y, z, dy/dx, position) per tracklet
 //   a3  (in gather_store) first sorted position of every bin (plus sentinel), z extent of every row
 //
+// Large loads take a counting sort instead of the radix passes (same result): the key kernel also counts every
+// bin, one inclusive scan turns the counts into first positions, place_tracklets puts every tracklet at the next
+// free position of its bin (atomic cursor = the table itself, which ends as the first-position table), and
+// order_bins restores the caller's order inside every bin (insertion sort by position, one thread per bin) and
+// records the z extents.  A bin longer than kMaxBin sets a device flag: the counting kernels after it return at
+// once and the radix kernels, enqueued behind them and gated on the same flag, do the work -- no host round trip.
+//
 // north_star: "device-side sort and index by chamber and local-y bin ... a radix sort plus
 // per-chamber y-bin offsets"; the 18 x 5 x 6 segmentation is PAPER.md:50.  The key also
 // carries the z row (SURVEY.md 8(d).3 "design consequence"), and it uses (sector, layer)
@@ -26,29 +33,47 @@ constexpr int kTile = kSortThreads * kItems;        // 4096 keys per tile
 
 // also packs (y, z, dy/dx, chamber) into one 16-byte record so that the gather after the sort reads
 // one sector per tracklet instead of three
+constexpr int kKeyItems = 8;                        // tracklets per thread
 __global__ void __launch_bounds__(256) tracklet_key(const float* __restrict__ y, const float* __restrict__ z,
                                                     const float* __restrict__ dydx, const int32_t* __restrict__ chamber,
                                                     const int32_t* __restrict__ interaction, uint32_t* __restrict__ key,
-                                                    float4* __restrict__ packed, int64_t n, IndexGeom g) {
-    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    const float yy = y[i], zz = z[i];
-    packed[i] = make_float4(yy, zz, dydx[i], __int_as_float(chamber[i]));
-    const int ch = chamber[i];
-    uint32_t k = g.n_bins;                          // unusable: behind every bin
-    const int ia = (g.n_ia > 1) ? interaction[i] : 0;      // time-frame association: the interaction leads the key
-    if (ch >= 0 && ch < g.n_chambers && isfinite(yy) && isfinite(zz) && ia >= 0 && ia < g.n_ia) {
-        const int sector = ch / g.per_sector, layer = ch % g.n_layers;
-        const uint32_t cell = (uint32_t)((ia * g.n_sectors + sector) * g.n_layers + layer);
-        k = ((cell * (uint32_t)g.nz + (uint32_t)zrow_of(g, zz)) << g.nb_shift) + (uint32_t)ybin_of(g, yy);
+                                                    float4* __restrict__ packed, int64_t n, IndexGeom g,
+                                                    uint32_t* __restrict__ digit_tot, int shift) {
+    // digit_tot (counting sort): how many keys carry each leading digit, for the partition that follows
+    __shared__ uint32_t cnt[kRadix];
+    if (digit_tot) {
+        cnt[threadIdx.x] = 0;
+        __syncthreads();
     }
-    key[i] = k;
+#pragma unroll
+    for (int u = 0; u < kKeyItems; ++u) {
+        const int64_t i = ((int64_t)blockIdx.x * kKeyItems + u) * 256 + threadIdx.x;
+        if (i >= n) break;
+        const float yy = y[i], zz = z[i];
+        const int ch = chamber[i];
+        packed[i] = make_float4(yy, zz, dydx[i], __int_as_float(ch));
+        uint32_t k = g.n_bins;                          // unusable: behind every bin
+        const int ia = (g.n_ia > 1) ? interaction[i] : 0;      // time-frame association: the interaction leads the key
+        if (ch >= 0 && ch < g.n_chambers && isfinite(yy) && isfinite(zz) && ia >= 0 && ia < g.n_ia) {
+            const int sector = ch / g.per_sector, layer = ch % g.n_layers;
+            const uint32_t cell = (uint32_t)((ia * g.n_sectors + sector) * g.n_layers + layer);
+            k = ((cell * (uint32_t)g.nz + (uint32_t)zrow_of(g, zz)) << g.nb_shift) + (uint32_t)ybin_of(g, yy);
+        }
+        key[i] = k;
+        if (digit_tot) atomicAdd(&cnt[(k >> shift) & (kRadix - 1)], 1u);
+    }
+    if (digit_tot) {
+        __syncthreads();
+        if (cnt[threadIdx.x]) atomicAdd(digit_tot + threadIdx.x, cnt[threadIdx.x]);
+    }
 }
 
 // per-tile histogram of one digit; hist[d * n_tiles + tile]
+// gate: when given, the kernel runs only if *gate != 0 (the counting sort gave up, see the header)
 __global__ void __launch_bounds__(kSortThreads) radix_hist(const uint32_t* __restrict__ key, uint32_t* __restrict__ hist,
-                                                           int64_t n, int n_tiles, int shift) {
+                                                           int64_t n, int n_tiles, int shift, const int* __restrict__ gate) {
     __shared__ uint32_t cnt[kRadix];
+    if (gate && *gate == 0) return;
     cnt[threadIdx.x] = 0;
     __syncthreads();
     const int64_t base = (int64_t)blockIdx.x * kTile;
@@ -88,9 +113,10 @@ __device__ inline uint32_t block_exclusive_scan(uint32_t v, uint32_t* warp_sums,
 
 // one block per digit: exclusive scan of that digit's counts over the tiles, total to digit_tot[d]
 __global__ void __launch_bounds__(kSortThreads) radix_rowscan(uint32_t* __restrict__ hist, uint32_t* __restrict__ digit_tot,
-                                                              int n_tiles) {
+                                                              int n_tiles, const int* __restrict__ gate) {
     __shared__ uint32_t warp_sums[32];
     __shared__ uint32_t total;
+    if (gate && *gate == 0) return;
     uint32_t* row = hist + (size_t)blockIdx.x * n_tiles;
     uint32_t carry = 0;
     for (int t0 = 0; t0 < n_tiles; t0 += kSortThreads) {
@@ -112,8 +138,9 @@ __global__ void __launch_bounds__(kSortThreads, 3) radix_scatter(const uint32_t*
                                                               uint32_t* __restrict__ key_out, uint32_t* __restrict__ val_out,
                                                               const uint32_t* __restrict__ hist,
                                                               const uint32_t* __restrict__ digit_tot, int64_t n, int n_tiles,
-                                                              int shift) {
+                                                              int shift, const int* __restrict__ gate) {
     __shared__ uint32_t warp_cnt[kSortWarps][kRadix];
+    if (gate && *gate == 0) return;
     __shared__ uint32_t digit_base[kRadix];    // global position of the tile's first key with digit d
     __shared__ uint32_t tile_off[kRadix];      // position inside the reordered tile of its first key with digit d
     __shared__ uint32_t s_key[kTile], s_val[kTile];
@@ -192,6 +219,90 @@ __global__ void __launch_bounds__(kSortThreads, 3) radix_scatter(const uint32_t*
     }
 }
 
+// First step of the counting sort: partition by the leading digit of the key, the tracklet itself travelling along
+// (rec_out gets (y, z, dy/dx, position), dx_out the radial offset of its chamber), every bin counted on the way
+// (count[key + 2]: the inclusive scan leaves first(k) at [k + 1]), so that the placement that follows finds the
+// tracklets of one bucket, and their bins, close together in L2.  The order inside a bucket is free (order_bins
+// restores the caller's order), hence no stable ranking: ranks inside the tile and the tile's place inside the bucket
+// come from atomic counters; the tile is reordered in shared memory so that the global writes are runs per digit.
+struct Partition {
+    const float4* packed;
+    float4* rec_out;
+    const float* chamber_dx;
+    float* dx_out;
+    uint32_t* count;
+    int n_chambers;
+};
+constexpr int kPartItems = 8;
+constexpr int kPartTile = 256 * kPartItems;
+constexpr size_t kPartSmem = (size_t)kPartTile * (sizeof(float4) + 2 * sizeof(uint32_t));
+
+__global__ void __launch_bounds__(256) partition_tracklets(const uint32_t* __restrict__ key_in, uint32_t* __restrict__ key_out,
+                                                           const Partition pl, const uint32_t* __restrict__ digit_tot,
+                                                           uint32_t* __restrict__ cursor, int64_t n, int shift) {
+    extern __shared__ float4 s_dyn[];
+    float4* const s_rec = s_dyn;
+    uint32_t* const s_key = reinterpret_cast<uint32_t*>(s_rec + kPartTile);
+    uint32_t* const s_pos = s_key + kPartTile;
+    __shared__ uint32_t s_cnt[kRadix], s_base[kRadix], s_off[kRadix];
+    __shared__ uint32_t warp_sums[32];
+    __shared__ uint32_t total;
+    s_cnt[threadIdx.x] = 0;
+    const uint32_t start = block_exclusive_scan(digit_tot[threadIdx.x], warp_sums, &total);     // syncs
+    const int64_t tile_base = (int64_t)blockIdx.x * kPartTile;
+    uint32_t k[kPartItems], rank[kPartItems];
+    float4 r[kPartItems];
+#pragma unroll
+    for (int u = 0; u < kPartItems; ++u) {
+        const int64_t i = tile_base + u * 256 + threadIdx.x;
+        k[u] = 0u;
+        r[u] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+        if (i < n) {
+            k[u] = key_in[i];
+            r[u] = pl.packed[i];
+        }
+    }
+#pragma unroll
+    for (int u = 0; u < kPartItems; ++u) {
+        rank[u] = 0u;
+        if (tile_base + u * 256 + threadIdx.x < n) rank[u] = atomicAdd(&s_cnt[(k[u] >> shift) & (kRadix - 1)], 1u);
+    }
+    __syncthreads();
+    const uint32_t c = s_cnt[threadIdx.x];
+    s_base[threadIdx.x] = start + (c ? atomicAdd(cursor + threadIdx.x, c) : 0u);
+    s_off[threadIdx.x] = block_exclusive_scan(c, warp_sums, &total);                             // syncs
+    __syncthreads();
+#pragma unroll
+    for (int u = 0; u < kPartItems; ++u) {
+        const int64_t i = tile_base + u * 256 + threadIdx.x;
+        if (i < n) {
+            const uint32_t lp = s_off[(k[u] >> shift) & (kRadix - 1)] + rank[u];
+            s_rec[lp] = r[u];
+            s_key[lp] = k[u];
+            s_pos[lp] = (uint32_t)i;
+        }
+    }
+    __syncthreads();
+    const int n_here = (int)min((int64_t)kPartTile, n - tile_base);
+#pragma unroll
+    for (int u = 0; u < kPartItems; ++u) {
+        const int j = u * 256 + threadIdx.x;
+        if (j < n_here) {
+            const uint32_t kk = s_key[j];
+            const uint32_t d = (kk >> shift) & (kRadix - 1);
+            const uint32_t dst = s_base[d] + ((uint32_t)j - s_off[d]);
+            const float4 tl = s_rec[j];
+            key_out[dst] = kk;
+            pl.rec_out[dst] = make_float4(tl.x, tl.y, tl.z, __uint_as_float(s_pos[j]));
+            if (pl.dx_out) {
+                const int ch = __float_as_int(tl.w);
+                pl.dx_out[dst] = (ch >= 0 && ch < pl.n_chambers) ? __ldg(pl.chamber_dx + ch) : 0.0f;
+            }
+            atomicAdd(pl.count + kk + 2, 1u);
+        }
+    }
+}
+
 __device__ __forceinline__ uint32_t ext_encode(float f) {          // order-preserving float -> uint
     const uint32_t b = __float_as_uint(f);
     return (b & 0x80000000u) ? ~b : (b ^ 0x80000000u);
@@ -206,7 +317,9 @@ __global__ void __launch_bounds__(256) gather_store(const uint32_t* __restrict__
                                                     const float4* __restrict__ packed, float4* __restrict__ store,
                                                     uint2* __restrict__ row_ext, int32_t* __restrict__ bin_first,
                                                     const float* __restrict__ chamber_dx, float* __restrict__ store_dx,
-                                                    int n_chambers, int64_t n, uint32_t n_bins, int nb_shift) {
+                                                    int n_chambers, int64_t n, uint32_t n_bins, int nb_shift,
+                                                    const int* __restrict__ gate) {
+    if (gate && *gate == 0) return;
     const int64_t base = (int64_t)blockIdx.x * (256 * kGather) + threadIdx.x;
     float4 tl[kGather];
     uint32_t k[kGather], kprev[kGather], p[kGather];
@@ -259,6 +372,170 @@ __global__ void __launch_bounds__(256) gather_store(const uint32_t* __restrict__
     }
 }
 
+// ---- counting sort of large loads (see the header) ---------------------------------------------------------------
+constexpr int kMaxBin = 32;                         // longest bin order_bins sorts; longer -> radix path
+constexpr int kScanItems = 16;
+constexpr int kScanChunk = 256 * kScanItems;        // table entries per block
+
+// sum of every chunk of the count table; flags a bin (entries 2 .. n_bins + 1; the unusable tracklets behind them
+// are never read and need no order) longer than kMaxBin
+__global__ void __launch_bounds__(256) count_reduce(const uint32_t* __restrict__ tab, uint32_t* __restrict__ partial, int64_t m,
+                                                    int64_t n_bins, int* __restrict__ flag) {
+    __shared__ uint32_t warp_sums[32];
+    __shared__ uint32_t total;
+    const int64_t base = (int64_t)blockIdx.x * kScanChunk + (int64_t)threadIdx.x * kScanItems;
+    uint32_t sum = 0, longest = 0;
+#pragma unroll
+    for (int q = 0; q < kScanItems / 4; ++q) {
+        const int64_t j = base + 4 * q;
+        uint32_t v[4] = {0u, 0u, 0u, 0u};
+        if (j + 3 < m) {
+            const uint4 t = *reinterpret_cast<const uint4*>(tab + j);
+            v[0] = t.x; v[1] = t.y; v[2] = t.z; v[3] = t.w;
+        } else {
+#pragma unroll
+            for (int u = 0; u < 4; ++u)
+                if (j + u < m) v[u] = tab[j + u];
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            sum += v[u];
+            if (j + u >= 2 && j + u < n_bins + 2) longest = max(longest, v[u]);
+        }
+    }
+    if (longest > (uint32_t)kMaxBin) *flag = 1;
+    block_exclusive_scan(sum, warp_sums, &total);
+    if (threadIdx.x == 0) partial[blockIdx.x] = total;
+}
+
+// exclusive scan of the chunk sums, one block
+__global__ void __launch_bounds__(1024) count_scan_partials(uint32_t* __restrict__ partial, int n_chunks) {
+    __shared__ uint32_t warp_sums[32];
+    __shared__ uint32_t total;
+    uint32_t carry = 0;
+    for (int t0 = 0; t0 < n_chunks; t0 += 1024) {
+        const int t = t0 + threadIdx.x;
+        const uint32_t v = (t < n_chunks) ? partial[t] : 0u;
+        const uint32_t ex = block_exclusive_scan(v, warp_sums, &total);
+        if (t < n_chunks) partial[t] = carry + ex;
+        carry += total;
+        __syncthreads();
+    }
+}
+
+// inclusive scan of the table in place
+__global__ void __launch_bounds__(256) count_apply(uint32_t* __restrict__ tab, const uint32_t* __restrict__ partial, int64_t m) {
+    __shared__ uint32_t warp_sums[32];
+    __shared__ uint32_t total;
+    const int64_t base = (int64_t)blockIdx.x * kScanChunk + (int64_t)threadIdx.x * kScanItems;
+    uint32_t v[kScanItems];
+#pragma unroll
+    for (int q = 0; q < kScanItems / 4; ++q) {
+        const int64_t j = base + 4 * q;
+        if (j + 3 < m) {
+            const uint4 t = *reinterpret_cast<const uint4*>(tab + j);
+            v[4 * q] = t.x; v[4 * q + 1] = t.y; v[4 * q + 2] = t.z; v[4 * q + 3] = t.w;
+        } else {
+#pragma unroll
+            for (int u = 0; u < 4; ++u) v[4 * q + u] = (j + u < m) ? tab[j + u] : 0u;
+        }
+    }
+#pragma unroll
+    for (int u = 1; u < kScanItems; ++u) v[u] += v[u - 1];
+    const uint32_t off = partial[blockIdx.x] + block_exclusive_scan(v[kScanItems - 1], warp_sums, &total);
+#pragma unroll
+    for (int q = 0; q < kScanItems / 4; ++q) {
+        const int64_t j = base + 4 * q;
+        if (j + 3 < m) {
+            *reinterpret_cast<uint4*>(tab + j) = make_uint4(v[4 * q] + off, v[4 * q + 1] + off, v[4 * q + 2] + off, v[4 * q + 3] + off);
+        } else {
+#pragma unroll
+            for (int u = 0; u < 4; ++u)
+                if (j + u < m) tab[j + u] = v[4 * q + u] + off;
+        }
+    }
+}
+
+// every tracklet to the next free position of its bin.  tab[k + 1] starts as first(k) and ends as first(k + 1):
+// afterwards tab[b] = first sorted position whose key is >= b, the table the match kernel reads.
+// The input is partitioned by the leading key digit (partition_tracklets): the blocks running at one time work on a
+// few buckets, whose bins and store lines stay in L2 until they are complete.
+__global__ void __launch_bounds__(256) place_tracklets(const uint32_t* __restrict__ key, const float4* __restrict__ rec,
+                                                       const float* __restrict__ rec_dx, uint32_t* __restrict__ tab,
+                                                       float4* __restrict__ store, float* __restrict__ store_dx, int64_t n,
+                                                       const int* __restrict__ flag) {
+    if (*flag != 0) return;
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const uint32_t pos = atomicAdd(tab + key[i] + 1, 1u);      // one tracklet per thread: more per thread measured slower
+    store[pos] = rec[i];
+    if (store_dx) store_dx[pos] = rec_dx[i];
+}
+
+// one thread per bin: the caller's order inside the bin (what the stable radix sort gives; the match kernel breaks
+// score ties of duplicate tracklets by store position, reading R6), and the z extent of every (cell, z row)
+__global__ void __launch_bounds__(256) order_bins(const uint32_t* __restrict__ tab, float4* __restrict__ store,
+                                                  float* __restrict__ store_dx, uint2* __restrict__ row_ext, int64_t n_bins,
+                                                  int nb_shift, const int* __restrict__ flag) {
+    if (*flag != 0) return;
+    const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    uint32_t row = 0xffffffffu, zlo = 0xffffffffu, zhi = 0u;
+    if (b < n_bins) {
+        const uint32_t a = tab[b], e = tab[b + 1];
+        if (e > a) {
+            float4 prev = store[a];
+            row = (uint32_t)(b >> nb_shift);
+            zlo = zhi = ext_encode(prev.y);
+            for (uint32_t i = a + 1; i < e; ++i) {
+                float4 v = store[i];
+                const uint32_t z = ext_encode(v.y);
+                zlo = min(zlo, z);
+                zhi = max(zhi, z);
+                if (__float_as_uint(prev.w) > __float_as_uint(v.w)) {       // out of order: sink v
+                    const float dxv = store_dx ? store_dx[i] : 0.0f;
+                    uint32_t j = i;
+                    while (j > a) {
+                        const float4 u = store[j - 1];
+                        if (__float_as_uint(u.w) < __float_as_uint(v.w)) break;
+                        store[j] = u;
+                        if (store_dx) store_dx[j] = store_dx[j - 1];
+                        --j;
+                    }
+                    store[j] = v;
+                    if (store_dx) store_dx[j] = dxv;
+                    v = store[i];
+                }
+                prev = v;
+            }
+        }
+    }
+    if (!row_ext) return;
+    const uint32_t row0 = __reduce_min_sync(0xffffffffu, row);      // empty bins carry 0xffffffff and neutral extents
+    if (__all_sync(0xffffffffu, row == row0 || row == 0xffffffffu)) {
+        zlo = __reduce_min_sync(0xffffffffu, zlo);
+        zhi = __reduce_max_sync(0xffffffffu, zhi);
+        if ((threadIdx.x & 31) == 0 && row0 != 0xffffffffu) {
+            atomicMin(&row_ext[row0].x, zlo);
+            atomicMax(&row_ext[row0].y, zhi);
+        }
+    } else if (row != 0xffffffffu) {
+        atomicMin(&row_ext[row].x, zlo);
+        atomicMax(&row_ext[row].y, zhi);
+    }
+}
+
+// trd_copy_index after a counting sort: the sorted positions and keys the radix path leaves behind
+__global__ void __launch_bounds__(256) export_sorted(const float4* __restrict__ store, const uint32_t* __restrict__ key,
+                                                     uint32_t* __restrict__ sorted_pos, uint32_t* __restrict__ sorted_key, int64_t n) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const uint32_t p = __float_as_uint(store[i].w);
+    sorted_pos[i] = p;
+    sorted_key[i] = key[p];
+}
+
+constexpr int64_t kCountingMin = 1 << 18;           // index_sort = 0: loads of at least this many tracklets are counting-sorted
+
 inline int ceil_log2(uint64_t v) {
     int b = 0;
     while ((1ull << b) < v) ++b;
@@ -293,7 +570,7 @@ int radix_tiles(int64_t n) { return (int)((n + kTile - 1) / kTile); }
 // key0/val0 and key1/val1 ping-pong; *side tells which pair holds the result.
 cudaError_t radix_sort_pairs(uint32_t* key0, uint32_t* key1, uint32_t* val0, uint32_t* val1, uint32_t* tile_hist,
                              uint32_t* digit_tot, int64_t n, int n_passes, cudaStream_t stream, int* side_out,
-                             int64_t* launches) {
+                             int64_t* launches, const int* gate) {
     const int n_tiles = radix_tiles(n);
     uint32_t* key[2] = {key0, key1};
     uint32_t* val[2] = {val0, val1};
@@ -302,15 +579,33 @@ cudaError_t radix_sort_pairs(uint32_t* key0, uint32_t* key1, uint32_t* val0, uin
         const int sh = p * kRadixBits;
         const uint32_t* kin = key[side];
         const uint32_t* vin = (p == 0) ? nullptr : val[side];
-        radix_hist<<<n_tiles, kSortThreads, 0, stream>>>(kin, tile_hist, n, n_tiles, sh);
-        radix_rowscan<<<kRadix, kSortThreads, 0, stream>>>(tile_hist, digit_tot, n_tiles);
+        radix_hist<<<n_tiles, kSortThreads, 0, stream>>>(kin, tile_hist, n, n_tiles, sh, gate);
+        radix_rowscan<<<kRadix, kSortThreads, 0, stream>>>(tile_hist, digit_tot, n_tiles, gate);
         radix_scatter<<<n_tiles, kSortThreads, 0, stream>>>(kin, vin, key[side ^ 1], val[side ^ 1], tile_hist, digit_tot, n,
-                                                           n_tiles, sh);
+                                                           n_tiles, sh, gate);
         *launches += 3;
         side ^= 1;
     }
     *side_out = side;
     return cudaGetLastError();
+}
+
+// trd_copy_index: sorted positions and keys into val[sorted_side] / key[sorted_side] when the counting sort built the store
+cudaError_t export_sorted_index(trd_handle* h, cudaStream_t stream) {
+    if (h->sort_kind != 1 || h->n_tracklets == 0) return cudaSuccess;
+    int flag = 0;
+    TRD_TRY(cudaMemcpyAsync(&flag, h->sort_flag.p, sizeof(int), cudaMemcpyDeviceToHost, stream));
+    TRD_TRY(cudaStreamSynchronize(stream));
+    if (flag != 0) {                                   // a bin was too long: the radix kernels did the work
+        h->sort_kind = 2;
+        return cudaSuccess;
+    }
+    const int64_t n = h->n_tracklets;
+    h->sorted_side = 1;
+    export_sorted<<<(unsigned)((n + 255) / 256), 256, 0, stream>>>((const float4*)h->store.p, (const uint32_t*)h->key[0].p,
+                                                                  (uint32_t*)h->val[1].p, (uint32_t*)h->key[1].p, n);
+    TRD_TRY(cudaGetLastError());
+    return cudaStreamSynchronize(stream);
 }
 
 cudaError_t build_index(trd_handle* h, const float* d_y, const float* d_z, const float* d_dydx,
@@ -350,7 +645,11 @@ cudaError_t build_index(trd_handle* h, const float* d_y, const float* d_z, const
     h->n_tracklets = n;
     h->index_loaded = false;
 
-    TRD_TRY(reserve(h->bin_first, ((size_t)g.n_bins + 1) * sizeof(int32_t), stream));
+    // counting sort: when asked for, or for loads large enough that the radix passes cost more than its extra launches
+    const bool counting = c.index_sort > 0 || (c.index_sort == 0 && n >= kCountingMin);
+    h->sort_kind = counting ? 1 : 0;
+    const size_t n_tab = (size_t)g.n_bins + 3;           // counts live at [key + 2] (see tracklet_key)
+    TRD_TRY(reserve(h->bin_first, n_tab * sizeof(int32_t), stream));
     // z extents per row only without association (with it a row holds a couple of tracklets and the table would be large)
     h->use_row_ext = g.n_ia == 1;
     if (h->use_row_ext) {
@@ -361,7 +660,8 @@ cudaError_t build_index(trd_handle* h, const float* d_y, const float* d_z, const
         TRD_TRY(cudaMemset2DAsync((char*)h->row_ext.p + sizeof(uint32_t), sizeof(uint2), 0x00, sizeof(uint32_t), n_rows, stream));
     }
     if (n == 0) {
-        TRD_TRY(cudaMemsetAsync(h->bin_first.p, 0, ((size_t)g.n_bins + 1) * sizeof(int32_t), stream));
+        TRD_TRY(cudaMemsetAsync(h->bin_first.p, 0, n_tab * sizeof(int32_t), stream));
+        h->sort_kind = 0;
         h->index_loaded = true;
         return cudaSuccess;
     }
@@ -375,20 +675,57 @@ cudaError_t build_index(trd_handle* h, const float* d_y, const float* d_z, const
         TRD_TRY(reserve(h->val[s], (size_t)n * sizeof(uint32_t), stream));
     }
     TRD_TRY(reserve(h->tile_hist, (size_t)kRadix * n_tiles * sizeof(uint32_t), stream));
-    TRD_TRY(reserve(h->digit_tot, kRadix * sizeof(uint32_t), stream));
+    TRD_TRY(reserve(h->digit_tot, 2 * kRadix * sizeof(uint32_t), stream));
 
-    const unsigned n_blk = (unsigned)((n + 255) / 256);
-    tracklet_key<<<n_blk, 256, 0, stream>>>(d_y, d_z, d_dydx, d_chamber, d_interaction, (uint32_t*)h->key[0].p,
-                                            (float4*)h->packed.p, n, g);
+    const int* gate = nullptr;
+    // the counting sort first partitions by the leading digit of the key
+    const int sh = h->key_bits > kRadixBits ? h->key_bits - kRadixBits : 0;
+    if (counting) TRD_TRY(cudaMemsetAsync(h->digit_tot.p, 0, 2 * kRadix * sizeof(uint32_t), stream));   // totals, cursors
+    tracklet_key<<<(unsigned)((n + 256 * kKeyItems - 1) / (256 * kKeyItems)), 256, 0, stream>>>(
+        d_y, d_z, d_dydx, d_chamber, d_interaction, (uint32_t*)h->key[0].p, (float4*)h->packed.p, n, g,
+        counting ? (uint32_t*)h->digit_tot.p : nullptr, sh);
     h->launches++;
+    if (counting) {
+        const int n_chunks = (int)((n_tab + kScanChunk - 1) / kScanChunk);
+        TRD_TRY(reserve(h->sort_flag, sizeof(int), stream));
+        TRD_TRY(reserve(h->scan_partial, (size_t)n_chunks * sizeof(uint32_t), stream));
+        TRD_TRY(reserve(h->part_rec, (size_t)n * sizeof(float4), stream));
+        if (has_dx) TRD_TRY(reserve(h->part_dx, (size_t)n * sizeof(float), stream));
+        TRD_TRY(cudaMemsetAsync(h->sort_flag.p, 0, sizeof(int), stream));
+        TRD_TRY(cudaMemsetAsync(h->bin_first.p, 0, n_tab * sizeof(uint32_t), stream));
+        uint32_t* tab = (uint32_t*)h->bin_first.p;
+        int* flag = (int*)h->sort_flag.p;
+        Partition pl;
+        pl.packed = (const float4*)h->packed.p;
+        pl.rec_out = (float4*)h->part_rec.p;
+        pl.chamber_dx = has_dx ? (const float*)h->chamber_dx.p : nullptr;
+        pl.dx_out = has_dx ? (float*)h->part_dx.p : nullptr;
+        pl.count = tab;
+        pl.n_chambers = g.n_chambers;
+        TRD_TRY(cudaFuncSetAttribute(partition_tracklets, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kPartSmem));
+        partition_tracklets<<<(unsigned)((n + kPartTile - 1) / kPartTile), 256, kPartSmem, stream>>>(
+            (const uint32_t*)h->key[0].p, (uint32_t*)h->key[1].p, pl, (const uint32_t*)h->digit_tot.p, (uint32_t*)h->digit_tot.p + kRadix, n, sh);
+        count_reduce<<<n_chunks, 256, 0, stream>>>(tab, (uint32_t*)h->scan_partial.p, (int64_t)n_tab, (int64_t)g.n_bins, flag);
+        count_scan_partials<<<1, 1024, 0, stream>>>((uint32_t*)h->scan_partial.p, n_chunks);
+        count_apply<<<n_chunks, 256, 0, stream>>>(tab, (const uint32_t*)h->scan_partial.p, (int64_t)n_tab);
+        place_tracklets<<<(unsigned)((n + 255) / 256), 256, 0, stream>>>((const uint32_t*)h->key[1].p, (const float4*)h->part_rec.p,
+                                                                         has_dx ? (const float*)h->part_dx.p : nullptr, tab, (float4*)h->store.p,
+                                                                         has_dx ? (float*)h->store_dx.p : nullptr, n, flag);
+        order_bins<<<(unsigned)(((int64_t)g.n_bins + 255) / 256), 256, 0, stream>>>(tab, (float4*)h->store.p, has_dx ? (float*)h->store_dx.p : nullptr,
+                                                                                    h->use_row_ext ? (uint2*)h->row_ext.p : nullptr,
+                                                                                    (int64_t)g.n_bins, g.nb_shift, flag);
+        h->launches += 6;
+        TRD_TRY(cudaGetLastError());
+        gate = flag;                                     // the radix kernels below run only if a bin was too long
+    }
     int side = 0;
     TRD_TRY(radix_sort_pairs((uint32_t*)h->key[0].p, (uint32_t*)h->key[1].p, (uint32_t*)h->val[0].p, (uint32_t*)h->val[1].p,
-                             (uint32_t*)h->tile_hist.p, (uint32_t*)h->digit_tot.p, n, h->n_passes, stream, &side, &h->launches));
+                             (uint32_t*)h->tile_hist.p, (uint32_t*)h->digit_tot.p, n, h->n_passes, stream, &side, &h->launches, gate));
     h->sorted_side = side;
     gather_store<<<(unsigned)((n + 256 * kGather - 1) / (256 * kGather)), 256, 0, stream>>>((const uint32_t*)h->val[side].p, (const uint32_t*)h->key[side].p,
                                            (const float4*)h->packed.p, (float4*)h->store.p, h->use_row_ext ? (uint2*)h->row_ext.p : nullptr,
                                            (int32_t*)h->bin_first.p, has_dx ? (const float*)h->chamber_dx.p : nullptr,
-                                           has_dx ? (float*)h->store_dx.p : nullptr, g.n_chambers, n, g.n_bins, g.nb_shift);
+                                           has_dx ? (float*)h->store_dx.p : nullptr, g.n_chambers, n, g.n_bins, g.nb_shift, gate);
     h->launches += 1;
     TRD_TRY(cudaGetLastError());
     h->index_loaded = true;

@@ -98,6 +98,11 @@ struct trd_handle {
     trd::Buffer chamber_dx; // float per chamber: radial offset from the nominal layer plane (trd_set_chamber_dx)
     trd::Buffer store_dx;   // float per sorted tracklet: the offset of its chamber (only when offsets are set)
     int sorted_side = 0;    // which of key[]/val[] holds the sorted result
+    int sort_kind = 0;      // last load: 0 = radix sort, 1 = counting sort, 2 = counting sort gave up (long bin), radix did it
+    trd::Buffer sort_flag;  // int: set by the counting sort when a bin is too long for it
+    trd::Buffer scan_partial;  // chunk sums of the count table
+    trd::Buffer part_rec;   // counting sort: float4 per tracklet, partitioned by the leading key digit
+    trd::Buffer part_dx;    // counting sort: chamber offset per partitioned tracklet (only when offsets are set)
     // staging for the *_host entry points
     trd::Buffer stage_tl;   // tracklets
     // pipelined host entry points (host_api.cu): own copy streams, a ring of staging slots
@@ -136,7 +141,9 @@ constexpr int kRecOut = 32;   // 6 idx | 5 par | 15 cov | x sector chi2 n_matche
 int radix_tiles(int64_t n);
 cudaError_t radix_sort_pairs(uint32_t* key0, uint32_t* key1, uint32_t* val0, uint32_t* val1, uint32_t* tile_hist,
                              uint32_t* digit_tot, int64_t n, int n_passes, cudaStream_t stream, int* side_out,
-                             int64_t* launches);
+                             int64_t* launches, const int* gate = nullptr);
+// after a counting sort: fills val[sorted_side] / key[sorted_side] for trd_copy_index (synchronises)
+cudaError_t export_sorted_index(trd_handle* h, cudaStream_t stream);
 // tracks.cu: SoA -> packed records + locality key; packed results -> SoA
 constexpr int kCountingBits = 16;     // track keys up to this many bits are counting-sorted (tracks.cu)
 int track_key_bits(const trd_handle* h);

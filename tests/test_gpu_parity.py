@@ -227,6 +227,27 @@ def test_track_binning_does_not_change_results(B, name):
     assert_parity(P.compare(on, want), want)
 
 
+@pytest.mark.parametrize("name,extra", [("central8", {}), ("pileup", dict(chamber_dx_sigma=0.3, res_model=1))])
+def test_index_sort_does_not_change_results(B, name, extra):
+    """trd_config.index_sort picks the device sort of trd_load_tracklets (index.cu): the store and therefore every
+    output are bit-identical with the radix passes and with the counting sort, also with displaced chambers (the
+    per-tracklet offsets travel with the store) and with every tracklet given twice (ties by the caller's order)."""
+    spec = dataclasses.replace(W.CONFIGS[name], **extra); d = W.generate(spec); cfg = W.matcher_config(spec)
+    want = O.match(cfg, d)
+    for dup in (False, True):
+        if dup:
+            d = dict(d, **{k: np.concatenate([d[k], d[k]]) for k in d if k.startswith("tl_")})
+        radix = run_gpu(B, dict(cfg, index_sort=-1), d)
+        counting = run_gpu(B, dict(cfg, index_sort=1), d)
+        for k in ("idx", "par", "cov", "x", "sector", "chi2", "n_matched", "n_evals"):
+            np.testing.assert_array_equal(counting[k], radix[k])
+        if dup:
+            n0 = d["tl_y"].shape[0] // 2
+            assert np.all(counting["idx"] < n0)                      # of two equal tracklets the first one given wins
+        else:
+            assert_parity(P.compare(counting, want, x_atol=1e-4 if extra else 0.0, par_atol=3e-5 if extra else P.PAR_ATOL), want)
+
+
 def test_pipelined_host_entry_points(B):
     """trd_match_host_async + trd_wait_host: nine batches through the four-slot ring (the fifth call has to
     retire the first), pinned and pageable buffers, two consecutive loads on one handle; bit-equal to the
