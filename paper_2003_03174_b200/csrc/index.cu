@@ -303,11 +303,6 @@ __global__ void __launch_bounds__(256) partition_tracklets(const uint32_t* __res
     }
 }
 
-__device__ __forceinline__ uint32_t ext_encode(float f) {          // order-preserving float -> uint
-    const uint32_t b = __float_as_uint(f);
-    return (b & 0x80000000u) ? ~b : (b ^ 0x80000000u);
-}
-
 // also records the z extent of every (cell, z row): row_ext[row] = (min, max) of the encoded z.  The keys are
 // sorted, so a warp almost always lies inside one row: one warp reduction and two atomics per warp.  Each
 // thread handles kGather tracklets (independent random 16-byte reads in flight), strided by the block size.
@@ -620,6 +615,7 @@ cudaError_t build_index(trd_handle* h, const float* d_y, const float* d_z, const
     g.nz = 2 * half_rows;
     g.z_off = (float)(half_rows * c.pad_length);
     g.inv_pad = (float)(1.0 / c.pad_length);
+    g.zrow_max = (float)(g.nz - 1);
     const double x_out = c.layer_x[c.n_layers - 1];
     const double y_half = x_out * tan(M_PI / c.n_sectors) * 1.02 + 1.0;
     int shift;
@@ -635,6 +631,7 @@ cudaError_t build_index(trd_handle* h, const float* d_y, const float* d_z, const
     if (shift > 10) shift = 10;
     while (shift > 0 && (uint64_t)n_cells * g.nz * (1ull << shift) >= (1ull << 28)) --shift;
     g.nb_shift = shift;
+    g.ybin_max = (float)((1 << shift) - 1);
     g.y_half = (float)y_half;
     g.inv_w = (float)((double)(1 << shift) / (2.0 * y_half));
     if ((uint64_t)n_cells * g.nz >= (1ull << 28)) return cudaErrorInvalidValue;     // too many interactions for the key

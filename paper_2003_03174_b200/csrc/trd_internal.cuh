@@ -4,6 +4,7 @@
 
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <string.h>
 
 #include <string>
 
@@ -20,19 +21,32 @@ struct IndexGeom {
     int nb_shift;      // log2(y bins per z row)
     float z_off, inv_pad;
     float y_half, inv_w;
+    float zrow_max, ybin_max;   // (float)(nz - 1), (float)(y bins per row - 1): the clamps of the two bin functions
     uint32_t n_bins;   // also the key of an unusable tracklet (sorts behind every bin)
 };
 
 __host__ __device__ inline int zrow_of(const IndexGeom& g, float z) {
     float f = floorf((z + g.z_off) * g.inv_pad);
-    f = fminf(fmaxf(f, 0.0f), (float)(g.nz - 1));
+    f = fminf(fmaxf(f, 0.0f), g.zrow_max);
     return (int)f;
 }
 
 __host__ __device__ inline int ybin_of(const IndexGeom& g, float y) {
     float f = floorf((y + g.y_half) * g.inv_w);
-    f = fminf(fmaxf(f, 0.0f), (float)((1 << g.nb_shift) - 1));
+    f = fminf(fmaxf(f, 0.0f), g.ybin_max);
     return (int)f;
+}
+
+// order-preserving float -> uint (the z extent of a row is kept by atomicMin / atomicMax on these, index.cu; the match
+// kernel compares the encoded bounds of its z window with them)
+__host__ __device__ inline uint32_t ext_encode(float f) {
+#ifdef __CUDA_ARCH__
+    const uint32_t b = __float_as_uint(f);
+#else
+    uint32_t b;
+    memcpy(&b, &f, sizeof b);
+#endif
+    return (b & 0x80000000u) ? ~b : (b ^ 0x80000000u);
 }
 
 // ---- constants of the match kernel, float32, derived in double on the host -------------------
