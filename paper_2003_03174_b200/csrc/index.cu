@@ -615,7 +615,8 @@ cudaError_t build_index(trd_handle* h, const float* d_y, const float* d_z, const
     g.nz = 2 * half_rows;
     g.z_off = (float)(half_rows * c.pad_length);
     g.inv_pad = (float)(1.0 / c.pad_length);
-    g.zrow_max = (float)(g.nz - 1);
+    g.z_bias = (float)((double)half_rows);
+    g.zrow_max = g.nz - 1;
     const double x_out = c.layer_x[c.n_layers - 1];
     const double y_half = x_out * tan(M_PI / c.n_sectors) * 1.02 + 1.0;
     int shift;
@@ -631,9 +632,10 @@ cudaError_t build_index(trd_handle* h, const float* d_y, const float* d_z, const
     if (shift > 10) shift = 10;
     while (shift > 0 && (uint64_t)n_cells * g.nz * (1ull << shift) >= (1ull << 28)) --shift;
     g.nb_shift = shift;
-    g.ybin_max = (float)((1 << shift) - 1);
+    g.ybin_max = (1 << shift) - 1;
     g.y_half = (float)y_half;
     g.inv_w = (float)((double)(1 << shift) / (2.0 * y_half));
+    g.y_bias = (float)((double)(1 << shift) / 2.0);
     if ((uint64_t)n_cells * g.nz >= (1ull << 28)) return cudaErrorInvalidValue;     // too many interactions for the key
     g.n_bins = (uint32_t)n_cells * (uint32_t)g.nz * (1u << shift);
     h->ybin_width = 2.0 * y_half / (double)(1 << shift);

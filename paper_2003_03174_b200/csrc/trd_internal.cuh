@@ -21,20 +21,19 @@ struct IndexGeom {
     int nb_shift;      // log2(y bins per z row)
     float z_off, inv_pad;
     float y_half, inv_w;
-    float zrow_max, ybin_max;   // (float)(nz - 1), (float)(y bins per row - 1): the clamps of the two bin functions
+    float z_bias, y_bias;       // z_off * inv_pad, y_half * inv_w: row = floor(z * inv_pad + z_bias), bin likewise
+    int zrow_max, ybin_max;     // nz - 1, y bins per row - 1: the clamps of the two bin functions
     uint32_t n_bins;   // also the key of an unusable tracklet (sorts behind every bin)
 };
 
-__host__ __device__ inline int zrow_of(const IndexGeom& g, float z) {
-    float f = floorf((z + g.z_off) * g.inv_pad);
-    f = fminf(fmaxf(f, 0.0f), g.zrow_max);
-    return (int)f;
+// Both bin functions are monotone in their argument and clamp, so a window query [lo, hi] covers every tracklet whose
+// coordinate lies in it; the index build and the match kernel share them.  One FFMA, one F2I.FLOOR, two integer clamps.
+__device__ __forceinline__ int zrow_of(const IndexGeom& g, float z) {
+    return min(max(__float2int_rd(fmaf(z, g.inv_pad, g.z_bias)), 0), g.zrow_max);
 }
 
-__host__ __device__ inline int ybin_of(const IndexGeom& g, float y) {
-    float f = floorf((y + g.y_half) * g.inv_w);
-    f = fminf(fmaxf(f, 0.0f), g.ybin_max);
-    return (int)f;
+__device__ __forceinline__ int ybin_of(const IndexGeom& g, float y) {
+    return min(max(__float2int_rd(fmaf(y, g.inv_w, g.y_bias)), 0), g.ybin_max);
 }
 
 // order-preserving float -> uint (the z extent of a row is kept by atomicMin / atomicMax on these, index.cu; the match
