@@ -212,6 +212,45 @@ def match(cfg: dict, data: dict, brute: bool = False, n_threads: int = 0, lo: in
     return out
 
 
+def match_alternatives(cfg: dict, data: dict, tracks, target_idx, eps: float = 1e-4, max_runs: int = 256) -> dict:
+    """Is the chain `target_idx[:, k]` a legitimate result for track `tracks[k]`?
+
+    The track is replayed with the decisions closer than `eps` (relative) to their threshold taken either way, until the
+    target chain comes out or `max_runs` replays are spent.  Returns `found` (number of replays, negative = not found)
+    and the outputs of the replay that reached the target, all with one column per selected track."""
+    y, z, d, ch = (np.ascontiguousarray(data[k]) for k in ("tl_y", "tl_z", "tl_dydx", "tl_chamber"))
+    par = np.ascontiguousarray(data["par"]); cov = np.ascontiguousarray(data["cov"])
+    x = np.ascontiguousarray(data["x"]); sec = np.ascontiguousarray(data["sector"])
+    assert par.dtype == np.float32 and cov.dtype == np.float32 and sec.dtype == np.int32
+    sel = np.ascontiguousarray(tracks, np.int64)
+    tgt = np.ascontiguousarray(target_idx, np.int32)
+    k = sel.shape[0]
+    assert tgt.shape == (6, k)
+    out = dict(found=np.zeros(k, np.int32), idx=np.zeros((6, k), np.int32), par=np.zeros((5, k)), cov=np.zeros((15, k)),
+               x=np.zeros(k), sector=np.zeros(k, np.int32), chi2=np.zeros(k), n_matched=np.zeros(k, np.int32),
+               n_evals=np.zeros(k, np.int32))
+    if k == 0:
+        return out
+    n_ia = int(data.get("n_interactions", 0) or 0)
+    if n_ia > 1:
+        tl_ia = np.ascontiguousarray(data["tl_interaction"]); trk_ia = np.ascontiguousarray(data["interaction"])
+        ia_args = (_ip(tl_ia), _ip(trk_ia), n_ia)
+    else:
+        ia_args = (None, None, 1)
+    dx = data.get("chamber_dx")
+    if dx is not None:
+        dx = np.ascontiguousarray(dx, np.float64)
+    rc = lib().orc_match_alternatives(
+        C.byref(make_config(cfg)), _fp(y), _fp(z), _fp(d), _ip(ch), C.c_int64(y.shape[0]), _fp(par), _fp(cov), _fp(x),
+        _ip(sec), C.c_int64(x.shape[0]), sel.ctypes.data_as(C.POINTER(C.c_int64)), C.c_int64(k), _ip(tgt),
+        C.c_double(eps), int(max_runs), _ip(out["found"]), _ip(out["idx"]), _dp(out["par"]), _dp(out["cov"]),
+        _dp(out["x"]), _ip(out["sector"]), _dp(out["chi2"]), _ip(out["n_matched"]), _ip(out["n_evals"]), *ia_args,
+        _dp(dx) if dx is not None else None)
+    if rc != 0:
+        raise RuntimeError(f"orc_match_alternatives failed: {rc}")
+    return out
+
+
 def refit(cfg: dict, data: dict, matched: dict, min_tracklets: int = 2) -> dict:
     """TRD-only inward refit of the chains in `matched` (the dict returned by match, or the CUDA path's output widened
     to float64) to the plane x_ref.  Returns par, cov, x, sector, chi2, n_used."""

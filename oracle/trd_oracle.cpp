@@ -33,6 +33,7 @@
 #include <cstdint>
 #include <cstring>
 #include <limits>
+#include <deque>
 #include <vector>
 #ifdef _OPENMP
 #include <omp.h>
@@ -93,11 +94,33 @@ inline double curvature_factor(const Config& cfg, double x, double y, double z) 
     return -0.00299792458 * cfg.bz_tesla * (1.0 + cfg.bz_r2 * (x * x + y * y) + cfg.bz_z2 * z * z);
 }
 
-inline void note(double* margin, double value, double threshold) {
+// ---- fragile decisions (R23: "several results are correct") ---------------------------
+// Every discrete decision of the algorithm compares a quantity with a threshold.  note() records the smallest relative
+// distance of any of them from its threshold: the per-track `margin`.  A float32 implementation may take a decision
+// whose distance is below its rounding the other way, and the result it then reaches is as legitimate as this one.
+// To check such a result (orc_match_alternatives) a track is replayed with chosen decisions taken the other way:
+// while a Replay is active, note() numbers the decisions closer than eps to their threshold in the order they are met
+// and returns true for those the replay flips.  Nothing else changes: with no Replay (every normal run) note() only
+// records the margin and returns false.
+constexpr int kMaxDecisions = 64;
+struct Replay {
+    double eps = 0.0;
+    int n_forced = 0;                           // decisions 0 .. n_forced-1 take forced[], later ones their natural outcome
+    unsigned char forced[kMaxDecisions] = {};   // 1 = the other way
+    int n_seen = 0;                             // fragile decisions met by the run
+};
+thread_local Replay* t_replay = nullptr;
+
+inline bool note(double* margin, double value, double threshold) {
     // relative distance of a quantity from the threshold it is compared with
-    if (!margin) return;
-    double m = std::fabs(value - threshold) / std::fabs(threshold);
-    if (m < *margin) *margin = m;
+    if (!margin && !t_replay) return false;
+    const double m = std::fabs(value - threshold) / std::fabs(threshold);
+    if (margin && m < *margin) *margin = m;
+    if (t_replay && m < t_replay->eps) {
+        const int k = t_replay->n_seen++;
+        if (k < t_replay->n_forced && k < kMaxDecisions) return t_replay->forced[k] != 0;
+    }
+    return false;
 }
 
 // (asin(w) - w) / w^2, with its series near 0
@@ -124,8 +147,8 @@ bool propagate_state(const Config& cfg, const double p[5], double x0, double x1,
     const double kappa = b * c;
     const double u = kappa * dx;
     const double f1 = s, f2 = s + u;
-    note(margin, std::fabs(f2), cfg.max_snp);
-    if (std::fabs(f1) >= 1.0 || std::fabs(f2) >= cfg.max_snp) return false;
+    const bool flip = note(margin, std::fabs(f2), cfg.max_snp);
+    if (std::fabs(f1) >= 1.0 || std::fabs(f2) >= 1.0 || ((std::fabs(f2) >= cfg.max_snp) != flip)) return false;
     const double r1 = std::sqrt(1.0 - f1 * f1), r2 = std::sqrt(1.0 - f2 * f2);
     const double cosd = r1 * r2 + f1 * f2;               // cos of the turning angle
     const double g = (1.0 + cosd) / (r1 + r2);
@@ -190,8 +213,8 @@ bool rotate_state(const Config& cfg, const double p[5], double x, double beta, d
     const double r = std::sqrt(1.0 - s * s);
     const double s2 = s * cb - r * sb;
     const double c2 = r * cb + s * sb;                    // cos(phi) in the new frame
-    note(margin, std::fabs(s2), cfg.max_snp);
-    if (std::fabs(s2) >= cfg.max_snp || c2 <= 0.0) return false;
+    const bool flip = note(margin, std::fabs(s2), cfg.max_snp);
+    if (std::fabs(s2) >= 1.0 || ((std::fabs(s2) >= cfg.max_snp) != flip) || c2 <= 0.0) return false;
     const double r2 = std::sqrt(1.0 - s2 * s2);
     *x_out = x * cb + y * sb;
     out[0] = -x * sb + y * cb;
@@ -247,8 +270,8 @@ bool apply_material(const Config& cfg, Hyp& h, int dir, double* margin) {
     const double dE = cfg.eloss * ell / beta2;
     const double E1 = E - dir * dE;
     if (dE > 0.0) {
-        note(margin, E1, cfg.mass);
-        if (E1 <= cfg.mass) return false;                       // stopped in the slab: state untouched
+        const bool flip = note(margin, E1, cfg.mass);
+        if ((E1 <= cfg.mass) != flip) return false;             // stopped in the slab: state untouched
     }
     const double th2 = 0.0136 * 0.0136 * cfg.x_over_x0 * ell / (beta2 * p2);
     h.C[2][2] += th2 * (1.0 - s * s) * (1.0 + t * t);
@@ -273,8 +296,8 @@ bool propagate_to_layer(const Config& cfg, Hyp& h, double X, double* margin, Cou
     const double edge = X * std::tan(half);
     if (!propagate(cfg, w, X, margin, cnt)) return false;
     for (int n_rot = 0;; ++n_rot) {
-        note(margin, std::fabs(w.p[0]), edge);
-        if (std::fabs(w.p[0]) <= edge) break;
+        const bool flip = note(margin, std::fabs(w.p[0]), edge);
+        if ((std::fabs(w.p[0]) <= edge) != flip) break;
         if (n_rot == 2) return false;
         const double beta = (w.p[0] > 0.0 ? 2.0 : -2.0) * half;
         if (!rotate(cfg, w, beta, margin, cnt)) return false;
@@ -426,20 +449,21 @@ void find_candidates(const Config& cfg, const Store& st, const Hyp& h, int layer
         const double ry = tl.y - (h.p[0] + tl.dx * rd.tanphi), rz = tl.z - (h.p[1] + tl.dx * rd.zslope);   // [R29]
         const double ryc = ry - rd.tan_tilt * rz;                            // y corrected with the extrapolated z
         const double da = std::fabs(tl.dydx - rd.tanphi);
-        const bool in_y = std::fabs(ryc) <= rd.road_y, in_z = std::fabs(rz) <= rd.road_z;
-        const bool pass = da <= veto;                                       // PAPER.md:60, 4 sigma [R8]
+        bool in_y = std::fabs(ryc) <= rd.road_y, in_z = std::fabs(rz) <= rd.road_z;
+        bool pass = da <= veto;                                             // PAPER.md:60, 4 sigma [R8]
         const bool loose_y = std::fabs(ryc) <= rd.road_y * (1.0 + kLoose);
         const bool loose_z = std::fabs(rz) <= rd.road_z * (1.0 + kLoose);
         const bool loose_a = da <= veto * (1.0 + kLoose);
-        if (loose_z && loose_a) note(margin, std::fabs(ryc), rd.road_y);
-        if (loose_y && loose_a) note(margin, std::fabs(rz), rd.road_z);
-        if (loose_y && loose_z) note(margin, da, veto);
+        if (loose_z && loose_a && note(margin, std::fabs(ryc), rd.road_y)) in_y = !in_y;
+        if (loose_y && loose_a && note(margin, std::fabs(rz), rd.road_z)) in_z = !in_z;
+        if (loose_y && loose_z && note(margin, da, veto)) pass = !pass;
         const double c2 = chi2_of(rd, ry, rz);                              // y and z only
-        if (loose_y && loose_z && loose_a) note(margin, c2, cfg.chi2_cut);
+        bool cut = c2 >= cfg.chi2_cut;                                      // per-layer cut [R4]
+        if (loose_y && loose_z && loose_a && note(margin, c2, cfg.chi2_cut)) cut = !cut;
         if (!(in_y && in_z && pass)) continue;
         if (n_evals) (*n_evals)++;                                          // one "candidate evaluation"
         if (cnt) cnt->n_cand++;
-        if (c2 >= cfg.chi2_cut) continue;                                   // per-layer cut [R4]
+        if (cut) continue;
         out.push_back({tl.index, tl.y, tl.z, c2, tl.dx});
     }
 }
@@ -455,6 +479,18 @@ struct TrackResult {
     int n_evals;
     double margin;
 };
+
+// relative gap between two neighbours of the sorted child list, (b - a) / |b| with a <= b: recorded as a margin like
+// every other decision; returns true if a replay takes the two the other way round
+inline bool rank_gap(double* margin, double a, double b) {
+    const double m = (b - a) / std::max(std::fabs(b), 1e-300);
+    if (margin && m < *margin) *margin = m;
+    if (t_replay && m < t_replay->eps) {
+        const int k = t_replay->n_seen++;
+        if (k < t_replay->n_forced && k < kMaxDecisions) return t_replay->forced[k] != 0;
+    }
+    return false;
+}
 
 // one track through all layers; "only the best N_candidates
 // hypotheses are propagated", Fig. 2
@@ -488,16 +524,15 @@ void match_track(const Config& cfg, const Store& st, const Hyp& seed, TrackResul
             return a.tracklet < b.tracklet;
         });
         const int keep = std::min<int>(cfg.n_hyp, (int)children.size());
-        // ranking margins: the keep boundary at every layer, the winner at the last layer
+        // ranking margins: the keep boundary at every layer, the winner at the last layer; a replay may take either of
+        // two children whose scores are closer than eps
         if ((int)children.size() > keep) {
             const double a = children[keep - 1].score, b = children[keep].score;
-            const double m = (b - a) / std::max(std::fabs(b), 1e-300);
-            if (m < *mg) *mg = m;
+            if (rank_gap(mg, a, b)) std::swap(children[keep - 1], children[keep]);
         }
         if (L == cfg.n_layers - 1 && children.size() > 1) {
             const double a = children[0].score, b = children[1].score;
-            const double m = (b - a) / std::max(std::fabs(b), 1e-300);
-            if (m < *mg) *mg = m;
+            if (rank_gap(mg, a, b)) std::swap(children[0], children[1]);
         }
         next.clear();
         for (int k = 0; k < keep; ++k) {
@@ -522,8 +557,8 @@ void match_track(const Config& cfg, const Store& st, const Hyp& seed, TrackResul
                 h.chi2 += chi2inc;
                 h.idx[L] = c.tracklet;
                 h.n_matched++;
-                note(mg, std::fabs(h.p[2]), cfg.max_snp);
-                if (std::fabs(h.p[2]) >= cfg.max_snp) h.alive = false;     // kept, but only skips from now on
+                const bool flip = note(mg, std::fabs(h.p[2]), cfg.max_snp);
+                if ((std::fabs(h.p[2]) >= cfg.max_snp) != flip) h.alive = false;     // kept, but only skips from now on
             }
             next.push_back(h);
         }
@@ -708,6 +743,96 @@ int orc_match(const orc_config* cfg, const float* tl_y, const float* tl_z, const
     if (seconds) {
         seconds[0] = std::chrono::duration<double>(t1 - t0).count();
         seconds[1] = std::chrono::duration<double>(t2 - t1).count();
+    }
+    return 0;
+}
+
+// ---- "several results are correct": is a given chain one of them? ---------------------------
+// For each of the n_sel tracks sel[k] (positions in the track arrays) the target chain target_idx[l * n_sel + k] (what
+// another implementation attached) is looked for among the results this algorithm reaches when decisions closer than eps
+// (relative) to their threshold -- road edges, chi2 cut, inclination veto, sector edge, max_snp, a stopping particle,
+// the rank gaps at the keep boundary of every layer and between the two best chains at the end -- are taken either way.
+// The search replays the track with one more fragile decision flipped at a time (breadth first: the natural run, every
+// single flip, every pair, ...; every set visited once), until the chain appears or max_runs replays are spent.  out_found[k] = the
+// number of replays it took (1 = the natural result is the target), or minus the number spent if it never appeared.  The
+// other outputs hold the result of the replay that reached the target (of the natural run if none did), n_sel columns.
+namespace {
+
+bool same_chain(const Config& cfg, const Hyp& h, const int32_t* target, int64_t stride, int64_t k) {
+    for (int l = 0; l < cfg.n_layers; ++l)
+        if (h.idx[l] != target[l * stride + k]) return false;
+    return true;
+}
+
+bool search_alternatives(const Config& cfg, const Store& st, const Hyp& seed, const int32_t* target, int64_t stride, int64_t k,
+                         double eps, int& runs, int max_runs, TrackResult& res) {
+    // breadth first over the sets of flipped decisions: the natural run, then every single flip, then pairs, ...  A
+    // replay with the decisions d0 < d1 < ... flipped meets the same decisions up to its last flip as its parent did,
+    // so its children flip one more decision met after that one: every set is visited once.
+    std::deque<Replay> queue;
+    Replay root;
+    root.eps = eps;
+    queue.push_back(root);
+    while (!queue.empty() && runs < max_runs) {
+        Replay rp = queue.front();
+        queue.pop_front();
+        rp.n_seen = 0;
+        t_replay = &rp;
+        match_track(cfg, st, seed, res, nullptr);
+        t_replay = nullptr;
+        ++runs;
+        if (same_chain(cfg, res.best, target, stride, k)) return true;
+        const int n_seen = std::min(rp.n_seen, kMaxDecisions);
+        for (int d = rp.n_forced; d < n_seen && (int)queue.size() < max_runs; ++d) {
+            Replay child = rp;
+            for (int q = rp.n_forced; q < d; ++q) child.forced[q] = 0;
+            child.forced[d] = 1;
+            child.n_forced = d + 1;
+            queue.push_back(child);
+        }
+    }
+    return false;
+}
+
+}  // namespace
+
+int orc_match_alternatives(const orc_config* cfg, const float* tl_y, const float* tl_z, const float* tl_dydx,
+                           const int32_t* tl_chamber, int64_t n_tl, const float* par, const float* cov, const float* x,
+                           const int32_t* sector, int64_t n_trk, const int64_t* sel, int64_t n_sel, const int32_t* target_idx,
+                           double eps, int max_runs, int32_t* out_found, int32_t* out_idx, double* out_par, double* out_cov,
+                           double* out_x, int32_t* out_sector, double* out_chi2, int32_t* out_n_matched, int32_t* out_n_evals,
+                           const int32_t* tl_ia, const int32_t* trk_ia, int32_t n_ia, const double* chamber_dx) {
+    if (cfg->n_layers > kMaxLayers || cfg->n_hyp < 1) return -1;
+    if ((tl_ia == nullptr) != (trk_ia == nullptr)) return -2;
+    Store st;
+    build_store(*cfg, tl_y, tl_z, tl_dydx, tl_chamber, tl_ia, n_ia, chamber_dx, n_tl, true, st);
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t k = 0; k < n_sel; ++k) {
+        const int64_t i = sel[k];
+        double p[5], c15[15];
+        for (int q = 0; q < 5; ++q) p[q] = par[q * n_trk + i];
+        for (int q = 0; q < 15; ++q) c15[q] = cov[q * n_trk + i];
+        Hyp seed;
+        load_hyp(seed, p, c15, x[i], sector[i]);
+        seed.ia = (st.n_ia > 1) ? trk_ia[i] : 0;
+        seed.alive = std::fabs(p[2]) < cfg->max_snp && sector[i] >= 0 && sector[i] < cfg->n_sectors;
+        TrackResult res;
+        int runs = 0;
+        const bool found = search_alternatives(*cfg, st, seed, target_idx, n_sel, k, eps, runs, max_runs, res);
+        if (!found) {                                            // report the natural result
+            match_track(*cfg, st, seed, res, nullptr);
+        }
+        out_found[k] = found ? runs : -runs;
+        const Hyp& b = res.best;
+        for (int l = 0; l < kMaxLayers; ++l) out_idx[l * n_sel + k] = (l < cfg->n_layers) ? b.idx[l] : -1;
+        for (int q = 0; q < 5; ++q) out_par[q * n_sel + k] = b.p[q];
+        store_cov(b, c15);
+        for (int q = 0; q < 15; ++q) out_cov[q * n_sel + k] = c15[q];
+        out_x[k] = b.x;
+        out_sector[k] = b.sector;
+        out_chi2[k] = b.chi2;
+        out_n_matched[k] = b.n_matched;
+        out_n_evals[k] = res.n_evals;
     }
     return 0;
 }

@@ -10,6 +10,11 @@ the per-track fragility `margin`).  Criteria (BASELINE.json north_star; DESIGN.m
   parameters  |got - want| <= 1e-4 |want| or <= 1e-5, on tracks with identical assignment;
   chi2        |got - want| <= 1e-3 |want| (+ chi2_atol), same tracks;
   integers    n_matched, sector, x exact on tracks with identical assignment.
+
+A track whose assignment differs (allowed only below `eps_margin`) is not skipped: `compare` lists it in
+`flip_tracks`, the caller asks the reference side whether the chain found here is one of the results its algorithm
+reaches when the decisions closer than `eps_margin` to their threshold are taken the other way, and
+`compare_alternatives` then applies the same numeric criteria against that alternative.
 """
 from __future__ import annotations
 
@@ -35,6 +40,7 @@ def compare(got: Dict[str, np.ndarray], want: Dict[str, np.ndarray], eps_margin:
     rep = dict(n_tracks=int(n), n_assign_mismatch=int(mism.sum()), n_fragile=int(fragile.sum()),
                n_unexplained=int((mism & ~fragile).sum()))
     rep["unexplained_tracks"] = np.nonzero(mism & ~fragile)[0][:20].tolist()
+    rep["flip_tracks"] = np.nonzero(mism & fragile)[0]            # to be validated with compare_alternatives
     rep["max_margin_of_mismatch"] = float(want["margin"][mism].max()) if mism.any() else 0.0
     s = same
     gp = got["par"][:, :n].astype(np.float64)
@@ -71,4 +77,25 @@ def compare(got: Dict[str, np.ndarray], want: Dict[str, np.ndarray], eps_margin:
         rep["n_evals_bad"] = int((s & ~fragile & (got["n_evals"][:n] != want["n_evals"])).sum())
     rep["ok"] = (rep["n_unexplained"] == 0 and rep["n_par_bad"] == 0 and rep["n_chi2_bad"] == 0
                  and rep["n_int_bad"] == 0 and rep["n_cov_bad"] == 0)
+    return rep
+
+
+def compare_alternatives(got: Dict[str, np.ndarray], alt: Dict[str, np.ndarray], tracks, chi2_atol: float = 0.0,
+                         cov_rtol: float = 2e-3, x_atol: float = 0.0, par_atol: float = PAR_ATOL) -> dict:
+    """The flipped tracks of `compare`: `alt` holds, for track tracks[k] in column k, the reference side's result
+    with its fragile decisions taken so that the chain of `got` comes out (`alt["found"][k]` > 0 if such a result
+    exists).  Every flip must be such an alternative, and parameters, chi2, covariance and integers must agree with
+    it under the same criteria as everywhere else."""
+    tracks = np.asarray(tracks, np.int64)
+    k = tracks.shape[0]
+    sub = {key: np.asarray(got[key])[..., tracks] for key in ("idx", "par", "cov", "x", "sector", "chi2", "n_matched")}
+    want = dict(alt)
+    want["margin"] = np.full(k, np.inf)               # nothing is exempt here: the chains must be identical
+    rep = compare(sub, want, chi2_atol=chi2_atol, cov_rtol=cov_rtol, x_atol=x_atol, par_atol=par_atol)
+    found = np.asarray(alt["found"]) > 0
+    rep["n_flips"] = int(k)
+    rep["n_not_an_alternative"] = int((~found).sum())
+    rep["not_an_alternative_tracks"] = tracks[~found][:20].tolist()
+    rep["max_replays"] = int(np.abs(np.asarray(alt["found"])).max()) if k else 0
+    rep["ok"] = bool(rep["ok"] and rep["n_not_an_alternative"] == 0 and rep["n_assign_mismatch"] == 0)
     return rep

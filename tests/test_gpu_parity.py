@@ -53,11 +53,41 @@ def run_gpu(B, cfg, data, batch=None, in_place=False):
         B.trd_destroy(h)
 
 
-def assert_parity(rep, want):
+FLIPS = []       # (what, tracks, fragile tracks, flipped chains) of every comparison of this session, printed at the end
+
+
+def check_parity(got, want, cfg, data, lo=0, what="", max_flip_frac=0.25, record=True, **tol):
+    """north_star criteria (parity.compare) + every flipped chain validated: on a track whose assignment differs the
+    oracle is asked whether the CUDA path's chain is one of the results it reaches itself when its decisions closer
+    than 1e-4 to their threshold are taken the other way (oracle.match_alternatives); if so, parameters, chi2,
+    covariance and integers are compared against THAT result under the same tolerances.  The number of flips is bounded:
+    measured 6-9 % of the fragile tracks on the five configs, at most 25 % (and never more than a
+    handful on small inputs) is accepted."""
+    rep = P.compare(got, want, **tol)
     assert rep["ok"], {k: v for k, v in rep.items()}
     assert rep["n_evals_bad"] == 0
-    # flips are only tolerated on fragile tracks, and there must be few of those
-    assert rep["n_assign_mismatch"] <= rep["n_fragile"]
+    flips = rep["flip_tracks"]
+    if record:
+        FLIPS.append((what, rep["n_tracks"], rep["n_fragile"], int(flips.shape[0])))
+    if flips.shape[0]:
+        n = want["x"].shape[0]
+        alt = O.match_alternatives(cfg, data, flips + lo, got["idx"][:, :n][:, flips], eps=P.EPS_MARGIN)
+        tol2 = {k: v for k, v in tol.items() if k != "eps_margin"}
+        rep2 = P.compare_alternatives({k: v[..., :n] for k, v in got.items()}, alt, flips, **tol2)
+        assert rep2["ok"], {k: v for k, v in rep2.items()}
+        assert flips.shape[0] <= max(3, max_flip_frac * rep["n_fragile"]), (flips.shape[0], rep["n_fragile"])
+    return rep
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _report_flips():
+    yield
+    tot = [sum(f[k] for f in FLIPS) for k in (1, 2, 3)]
+    print(f"\n[parity] {len(FLIPS)} comparisons, {tot[0]} tracks, {tot[1]} fragile (margin < 1e-4), {tot[2]} flipped chains, "
+          f"every one validated as an alternative result of the oracle")
+    for what, n, nf, nfl in FLIPS:
+        if what:
+            print(f"[parity] {what}: {n} tracks, {nf} fragile, {nfl} flips")
 
 
 @pytest.mark.parametrize("name", ["tiny", "central", "central8", "pileup"])
@@ -65,8 +95,7 @@ def test_configs_1_to_4_full_parity(B, name):
     spec = W.CONFIGS[name]; d = W.generate(spec); cfg = W.matcher_config(spec)
     want = O.match(cfg, d)
     got = run_gpu(B, cfg, d)
-    rep = P.compare(got, want)
-    assert_parity(rep, want)
+    rep = check_parity(got, want, cfg, d, what=f"config {name}")
     assert rep["n_fragile"] < 0.02 * spec.n_tracks
 
 
@@ -77,7 +106,7 @@ def test_config_5_scaled_down_in_batches(B):
     d = W.generate(spec); cfg = W.matcher_config(spec)
     want = O.match(cfg, d)
     got = run_gpu(B, cfg, d, batch=spec.batch // 4)
-    assert_parity(P.compare(got, want), want)
+    check_parity(got, want, cfg, d, what="config timeframe scaled to 100k tracks")
 
 
 def test_dense_candidates_many_per_road(B):
@@ -91,27 +120,27 @@ def test_dense_candidates_many_per_road(B):
         want = O.match(cfg, d)
         assert want["counters"]["n_cand"] > want["counters"]["n_road"]
         got = run_gpu(B, cfg, d)
-        rep = P.compare(got, want)
-        assert_parity(rep, want)
+        check_parity(got, want, cfg, d, what=f"dense noise, n_hyp {n_hyp}")
 
 
-def test_config_5_full_size_sampled(B):
+def test_config_5_full_size_every_track(B):
     """BASELINE.json configs[4] at full size in the launch configuration bench.py times (one load of all
-    ~18.8M tracklets, four trd_match calls of 500k tracks); the oracle checks a sample of the tracks one
-    by one against the full tracklet set."""
+    ~18.8M tracklets, four trd_match calls of 500k tracks): ALL 2,000,000 tracks are compared with the oracle, which
+    matches them in eight slices against the full tracklet set ("parity is still checked on all 2M
+    tracks"); every flipped chain is validated as everywhere else."""
     spec = W.CONFIGS["timeframe"]; d = W.generate(spec); cfg = W.matcher_config(spec)
     got = run_gpu(B, cfg, d, batch=spec.batch)
-    rng = np.random.default_rng(5)
-    starts = np.sort(rng.choice(spec.n_tracks - 2048, 8, replace=False))
-    n_checked = 0
-    for lo in starts.tolist() + [spec.n_tracks - 2048]:
-        hi = lo + 2048
+    n_checked = n_fragile = n_flips = 0
+    step = 250_000
+    for lo in range(0, spec.n_tracks, step):
+        hi = min(spec.n_tracks, lo + step)
         want = O.match(cfg, d, lo=lo, hi=hi)
         part = {k: v[..., lo:hi] for k, v in got.items()}
-        rep = P.compare(part, want)
-        assert_parity(rep, want)
-        n_checked += hi - lo
-    assert n_checked >= 18_000
+        rep = check_parity(part, want, cfg, d, lo=lo, record=False)
+        n_checked += hi - lo; n_fragile += rep["n_fragile"]; n_flips += int(rep["flip_tracks"].shape[0])
+        del want
+    assert n_checked == spec.n_tracks == 2_000_000
+    FLIPS.append(("config timeframe at full size", n_checked, n_fragile, n_flips))
     # properties that hold at any size
     att = got["idx"] >= 0
     assert np.array_equal(att.sum(axis=0), got["n_matched"])
@@ -129,19 +158,19 @@ def test_edge_cases(B, base_cfg):
     spec = W.CONFIGS["tiny"]; d = W.generate(spec); cfg = W.matcher_config(spec)
     want = O.match(cfg, d)
     # in-place outputs (out->par == in->par)
-    assert_parity(P.compare(run_gpu(B, cfg, d, in_place=True), want), want)
+    check_parity(run_gpu(B, cfg, d, in_place=True), want, cfg, d)
     # ragged batches
-    assert_parity(P.compare(run_gpu(B, cfg, d, batch=333), want), want)
+    check_parity(run_gpu(B, cfg, d, batch=333), want, cfg, d)
     # dead seeds: |sin(phi)| >= max_snp, sector outside 0..17
     d2 = dict(d); d2["par"] = d["par"].copy(); d2["par"][2, 0] = 0.96
     d2["sector"] = d["sector"].copy(); d2["sector"][1] = 99; d2["sector"][2] = -1
     want2 = O.match(cfg, d2); got2 = run_gpu(B, cfg, d2)
-    assert_parity(P.compare(got2, want2), want2)
+    check_parity(got2, want2, cfg, d2)
     assert got2["idx"][:, :3].max() == -1 and got2["n_matched"][:3].max() == 0
     # no tracklets at all: every layer skipped, state = last alive propagation
     d3 = dict(d); d3.update(tl_y=d["tl_y"][:0], tl_z=d["tl_z"][:0], tl_dydx=d["tl_dydx"][:0], tl_chamber=d["tl_chamber"][:0])
     want3 = O.match(cfg, d3); got3 = run_gpu(B, cfg, d3)
-    assert_parity(P.compare(got3, want3), want3)
+    check_parity(got3, want3, cfg, d3)
     assert got3["idx"].max() == -1 and np.all(got3["x"] >= 247.0)
     # zero tracks, and trd_match before any load
     h = B.trd_create(cfg)
@@ -182,7 +211,7 @@ def test_variants(B, variant):
         spec = dataclasses.replace(spec, pt_spectrum="exp")    # sector crossings, tracks that curl up
     d = W.generate(spec); cfg = dict(W.matcher_config(spec), **over)
     want = O.match(cfg, d); got = run_gpu(B, cfg, d)
-    assert_parity(P.compare(got, want), want)
+    check_parity(got, want, cfg, d, what=f"variant {variant}")
 
 
 def test_host_entry_points_equal_device_entry_points(B):
@@ -224,7 +253,7 @@ def test_track_binning_does_not_change_results(B, name):
         np.testing.assert_array_equal(on_inplace[k], off[k])
         np.testing.assert_array_equal(on_ragged[k], off[k])
     want = O.match(cfg, d)
-    assert_parity(P.compare(on, want), want)
+    check_parity(on, want, cfg, d)
 
 
 @pytest.mark.parametrize("name", ["central8", "pileup"])
@@ -238,8 +267,7 @@ def test_zero_penalty_scores_of_zero(B, name):
     # the output is the seed propagated through six layers without a single update: for the curling 0.3 GeV/c tracks of
     # the pile-up spectrum the float32 rounding of +-60 cm excursions in y stays in the state (4e-5 cm seen; the same
     # with integer key compares), hence the stress floor of DESIGN.md 5 instead of the configs' 1e-5
-    rep = P.compare(got, want, par_atol=1e-4)
-    assert_parity(rep, want)
+    rep = check_parity(got, want, cfg, d, par_atol=1e-4)
     assert rep["n_assign_mismatch"] == 0
     assert got["n_matched"].max() == 0                                # nothing beats a chain of free skips
 
@@ -262,7 +290,7 @@ def test_index_sort_does_not_change_results(B, name, extra):
             n0 = d["tl_y"].shape[0] // 2
             assert np.all(counting["idx"] < n0)                      # of two equal tracklets the first one given wins
         else:
-            assert_parity(P.compare(counting, want, x_atol=1e-4 if extra else 0.0, par_atol=3e-5 if extra else P.PAR_ATOL), want)
+            check_parity(counting, want, cfg, d, x_atol=1e-4 if extra else 0.0, par_atol=3e-5 if extra else P.PAR_ATOL)
 
 
 def test_pipelined_host_entry_points(B):
@@ -301,8 +329,8 @@ def test_resolution_model_and_pad_tilt(B, name, n_hyp):
     d = W.generate(spec); cfg = W.matcher_config(spec)
     assert cfg["res_model"] == 1 and cfg["tan_tilt"] > 0.03
     want = O.match(cfg, d)
-    assert_parity(P.compare(run_gpu(B, cfg, d), want), want)
-    assert_parity(P.compare(run_gpu(B, dict(cfg, track_binning=1), d, batch=1777), want), want)
+    check_parity(run_gpu(B, cfg, d), want, cfg, d, what=f"resolution model + pad tilt, {name}")
+    check_parity(run_gpu(B, dict(cfg, track_binning=1), d, batch=1777), want, cfg, d)
     # the model matters: the same input matched without the tilt loses tracklets
     plain = run_gpu(B, dict(cfg, tan_tilt=0.0), d)
     assert plain["n_matched"].sum() < 0.97 * want["n_matched"].sum()
@@ -314,7 +342,7 @@ def test_resolution_model_dense(B):
     d = W.generate(spec); cfg = W.matcher_config(spec)
     want = O.match(cfg, d)
     assert want["counters"]["n_cand"] > want["counters"]["n_road"]
-    assert_parity(P.compare(run_gpu(B, cfg, d), want), want)
+    check_parity(run_gpu(B, cfg, d), want, cfg, d, what="resolution model, dense noise")
 
 
 @pytest.mark.parametrize("name,n_ia,n_hyp", [("central", 4, 1), ("pileup", 5, 4), ("central8", 7, 8)])
@@ -325,8 +353,8 @@ def test_time_frame_association(B, name, n_ia, n_hyp):
     d = W.generate(spec); cfg = W.matcher_config(spec)
     want = O.match(cfg, d)
     got = run_gpu(B, cfg, d)
-    assert_parity(P.compare(got, want), want)
-    assert_parity(P.compare(run_gpu(B, dict(cfg, track_binning=1), d, batch=2111), want), want)
+    check_parity(got, want, cfg, d, what=f"time-frame association, {name}")
+    check_parity(run_gpu(B, dict(cfg, track_binning=1), d, batch=2111), want, cfg, d)
     att = got["idx"] >= 0                                     # every attached tracklet is of the track's interaction
     ia_tl = d["tl_interaction"][np.where(att, got["idx"], 0)]
     assert np.all(ia_tl[att] == np.broadcast_to(d["interaction"], att.shape)[att])
@@ -341,7 +369,7 @@ def test_time_frame_association_at_scale_and_bad_ids(B):
     d["tl_interaction"][::97] = 100
     want = O.match(cfg, d)
     got = run_gpu(B, cfg, d, batch=50_000)
-    assert_parity(P.compare(got, want), want)
+    check_parity(got, want, cfg, d, what="time-frame association, 200k tracks in 100 interactions")
     assert got["n_matched"][:3].max() == 0
     import torch
     h = B.trd_create(cfg)
@@ -369,8 +397,8 @@ def test_two_stage_propagation_with_displaced_chambers(B, name, n_hyp, extra):
     want = O.match(cfg, d)
     got = run_gpu(B, cfg, d)
     # one more float32 propagation per attached tracklet: the absolute floor of the stress sweep
-    assert_parity(P.compare(got, want, x_atol=1e-4, par_atol=3e-5), want)
-    assert_parity(P.compare(run_gpu(B, dict(cfg, track_binning=1), d, batch=1999), want, x_atol=1e-4, par_atol=3e-5), want)
+    check_parity(got, want, cfg, d, what=f"two-stage propagation, {name}", x_atol=1e-4, par_atol=3e-5)
+    check_parity(run_gpu(B, dict(cfg, track_binning=1), d, batch=1999), want, cfg, d, x_atol=1e-4, par_atol=3e-5)
     assert np.abs(got["x"] - 364.0).max() > 0.3                       # states live at the displaced radii
     # the offsets matter, and clearing them gives the plain matcher again
     plain_want = O.match(cfg, {k: v for k, v in d.items() if k != "chamber_dx"})
@@ -389,7 +417,7 @@ def test_two_stage_propagation_with_displaced_chambers(B, name, n_hyp, extra):
     finally:
         B.trd_destroy(h)
     no_dx = {k: v for k, v in d.items() if k != "chamber_dx"}
-    assert_parity(P.compare(run_gpu(B, cfg, no_dx), plain_want), plain_want)
+    check_parity(run_gpu(B, cfg, no_dx), plain_want, cfg, no_dx)
 
 
 MATERIAL = dict(x_over_x0=W.X_OVER_X0, eloss=W.ELOSS, eloss_fluct=W.ELOSS_FLUCT)
@@ -409,17 +437,17 @@ def test_material_scattering_and_energy_loss(B, name, n_hyp, extra):
     # the parameter tolerance is widened accordingly (1e-4 cm ~ 3e-4 sigma_y of such a track)
     tol = dict(par_atol=1e-4, **(dict(x_atol=1e-4) if spec.chamber_dx_sigma > 0 else {}))
     got = run_gpu(B, cfg, d)
-    assert_parity(P.compare(got, want, **tol), want)
-    assert_parity(P.compare(run_gpu(B, dict(cfg, track_binning=1), d, batch=1999), want, **tol), want)
+    check_parity(got, want, cfg, d, what=f"material, {name}", **tol)
+    check_parity(run_gpu(B, dict(cfg, track_binning=1), d, batch=1999), want, cfg, d, **tol)
     # the material matters on these inputs, and the filter without it is the plain one
     none = dict(cfg, x_over_x0=0.0, eloss=0.0)
     plain_want = O.match(none, d)
     assert plain_want["n_matched"].sum() < 0.99 * want["n_matched"].sum()
-    assert_parity(P.compare(run_gpu(B, none, d), plain_want, **tol), plain_want)
+    check_parity(run_gpu(B, none, d), plain_want, none, d, **tol)
     # scattering only / energy loss only
     for part in (dict(cfg, eloss=0.0), dict(cfg, x_over_x0=0.0)):
         w = O.match(part, d)
-        assert_parity(P.compare(run_gpu(B, part, d), w, **tol), w)
+        check_parity(run_gpu(B, part, d), w, part, d, **tol)
     for bad in (dict(cfg, x_over_x0=-1.0), dict(cfg, eloss=float("nan")), dict(cfg, mass=-0.1)):
         with pytest.raises(B.TrdError) as e:
             B.trd_create(bad)
@@ -441,17 +469,17 @@ def test_field_inhomogeneity(B, name, n_hyp, extra):
     # same floor as the material tests: 0.3 GeV/c tracks at |sin(phi)| ~ 0.9 in the outer layers (one of 25 000 at 3.7e-5 cm)
     tol = dict(par_atol=1e-4, **(dict(x_atol=1e-4) if spec.chamber_dx_sigma > 0 else {}))
     got = run_gpu(B, cfg, d)
-    assert_parity(P.compare(got, want, **tol), want)
-    assert_parity(P.compare(run_gpu(B, dict(cfg, track_binning=1), d, batch=1999), want, **tol), want)
+    check_parity(got, want, cfg, d, what=f"field inhomogeneity, {name}", **tol)
+    check_parity(run_gpu(B, dict(cfg, track_binning=1), d, batch=1999), want, cfg, d, **tol)
     # the inhomogeneity matters on these inputs (chi2 grows when it is ignored) and the uniform filter is the plain one
     uni = dict(cfg, bz_r2=0.0, bz_z2=0.0)
     plain_want = O.match(uni, d)
     m = (want["n_matched"] > 0) & (plain_want["n_matched"] == want["n_matched"])
     assert plain_want["chi2"][m].sum() > 1.005 * want["chi2"][m].sum()
-    assert_parity(P.compare(run_gpu(B, uni, d), plain_want, **tol), plain_want)
+    check_parity(run_gpu(B, uni, d), plain_want, uni, d, **tol)
     for part in (dict(cfg, bz_z2=0.0), dict(cfg, bz_r2=0.0)):
         w = O.match(part, d)
-        assert_parity(P.compare(run_gpu(B, part, d), w, **tol), w)
+        check_parity(run_gpu(B, part, d), w, part, d, **tol)
     for bad in (dict(cfg, bz_r2=float("inf")), dict(cfg, bz_r2=-1e-5)):
         with pytest.raises(B.TrdError) as e:
             B.trd_create(bad)
@@ -465,7 +493,7 @@ def test_material_stops_slow_particles(B):
     want = O.match(cfg, d)
     got = run_gpu(B, cfg, d)
     assert want["n_matched"].sum() == 0 and got["n_matched"].sum() == 0
-    assert_parity(P.compare(got, want), want)
+    check_parity(got, want, cfg, d)
     assert np.all(got["x"] == 300.0)                                  # reached the first plane, stopped in its slab
 
 
@@ -493,9 +521,8 @@ def test_random_configurations(B):
         # the five configs are held to the north_star's 1e-5
         # chi2_atol: a chain of ONE tracklet that sits 0.01 sigma from the track has chi2 ~ 1e-4, and the float32 rounding of
         # y ~ 30 cm (2e-6 cm) is then 1 % of its residual; the relative criterion needs an absolute floor there
-        rep = P.compare(got, want, x_atol=1e-4 if spec.chamber_dx_sigma > 0 else 0.0, chi2_atol=1e-5,
-                        par_atol=1e-4 if (spec.x_over_x0 > 0 or spec.bz_r2 != 0) else 3e-5)
-        assert rep["ok"] and rep["n_evals_bad"] == 0 and rep["n_assign_mismatch"] <= rep["n_fragile"], (k, spec, cfg, rep)
+        check_parity(got, want, cfg, d, x_atol=1e-4 if spec.chamber_dx_sigma > 0 else 0.0, chi2_atol=1e-5,
+                     par_atol=1e-4 if (spec.x_over_x0 > 0 or spec.bz_r2 != 0) else 3e-5)
 
 
 @pytest.mark.parametrize("name,extra", [("central", {}), ("pileup", dict(res_model=1, chamber_dx_sigma=0.3)), ("central8", {}),
