@@ -44,9 +44,9 @@ bool derive_params(const trd_config& c, trd::MatchParams& mp) {
     mp.b = (float)(-0.00299792458 * c.bz_tesla);
     const double cb = cos(2.0 * half), sb = sin(2.0 * half);
     mp.cb_hi = (float)cb;
-    mp.cb_lo = (float)(cb - (double)mp.cb_hi);
     mp.sb_hi = (float)sb;
-    mp.sb_lo = (float)(sb - (double)mp.sb_hi);
+    mp.cbd = cb;
+    mp.sbd = sb;
     mp.sig_y2 = (float)(c.sigma_y * c.sigma_y);
     mp.sig_z2 = (float)(c.sigma_z * c.sigma_z);
     mp.n_sigma_road = (float)c.n_sigma_road;

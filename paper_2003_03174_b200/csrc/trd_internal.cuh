@@ -55,7 +55,8 @@ struct MatchParams {
     float layer_x[TRD_MAX_LAYERS];
     float edge[TRD_MAX_LAYERS];      // layer_x * tan(pi / n_sectors): the sector edge in y
     float b;                         // kappa = b * q/pT
-    float cb_hi, cb_lo, sb_hi, sb_lo;  // cos / sin of the sector width, split hi + lo
+    float cb_hi, sb_hi;              // cos / sin of the sector width, float32 (Jacobian of the frame change)
+    double cbd, sbd;                 // the same in double (the point and sin(phi) in the new frame)
     float sig_y2, sig_z2;
     float n_sigma_road, half_pad;
     float veto;                      // n_sigma_angle * sigma_dydx
