@@ -41,7 +41,8 @@ bool derive_params(const trd_config& c, trd::MatchParams& mp) {
         mp.layer_x[l] = (float)c.layer_x[l];
         mp.edge[l] = (float)(c.layer_x[l] * tan(half));
     }
-    mp.b = (float)(-0.00299792458 * c.bz_tesla);
+    mp.bd = -0.00299792458 * c.bz_tesla;
+    mp.b = (float)mp.bd;
     const double cb = cos(2.0 * half), sb = sin(2.0 * half);
     mp.cb_hi = (float)cb;
     mp.sb_hi = (float)sb;

@@ -57,6 +57,7 @@ struct MatchParams {
     float b;                         // kappa = b * q/pT
     float cb_hi, sb_hi;              // cos / sin of the sector width, float32 (Jacobian of the frame change)
     double cbd, sbd;                 // the same in double (the point and sin(phi) in the new frame)
+    double bd;                       // b in double: sin(phi) advances by bd * q/pT * dx
     float sig_y2, sig_z2;
     float n_sigma_road, half_pad;
     float veto;                      // n_sigma_angle * sigma_dydx
