@@ -32,10 +32,13 @@ UNIT = "tracks/s"
 # Algorithmic flops per unit, counted from the formulas of DESIGN.md "Arithmetic" (= SURVEY.md 8(d).3):
 # FMA = 2, add/mul/compare = 1, div/sqrt = 1.  Units per launch come from the oracle's counters.
 FLOP = dict(n_prop=180, n_rot=60, n_road=25, n_cand=12, n_upd=110)
-BYTES_TRACK_IN = 88       # 5 + 15 floats, x, sector
-BYTES_TRACK_OUT = 124     # 6 indices, 5 + 15 floats, x, sector, chi2, n_matched, n_cand_evals
-BYTES_PER_CAND = 16       # one (y, z, dy/dx, position) store entry per candidate evaluation
+# Algorithmic bytes: a track in 88 B (5 + 15 floats, x, sector), out 120 B (6 indices, 5 + 15 floats, x,
+# sector, chi2, n_matched), every DISTINCT tracklet found inside some road once at 12 B (y, z, dy/dx).
+BYTES_TRACK_IN = 88
+BYTES_TRACK_OUT = 120
+BYTES_PER_CAND = 12
 ORACLE_SAMPLE_TRACKS = 200_000
+ORACLE_SAMPLE_TRACKS_1T = 20_000     # the one-thread leg of the oracle (Fig. 5 has both CPU curves)
 
 
 def fp32_peak_tflops(sm_count: int, sm_mhz: float) -> float:
@@ -113,11 +116,14 @@ def load_units(spec, n_batches):
     return u["batches"]
 
 
-def load_bytes(info: dict, n_tl: int) -> float:
-    """Bytes trd_load_tracklets has to move with the sort it used: the radix path reads the SoA (16),
-    writes record + key (20), per pass 4 + 8 + 8, then gathers (4 + 4 + 16 + 16); the counting path reads the SoA (16),
-    writes record + key (20), partitions (20 + 20), places (20 + 16), orders (16) and passes five times over the
-    4-byte bin table."""
+def load_bytes_algorithmic(info: dict, n_tl: int) -> float:
+    """SURVEY.md 8(d).3, tracklet load + sort + index per tracklet: 16 B in + (8 B + 8 B) per 8-bit pass over the key +
+    12 B gather + 16 B out = 44 + 16 x passes (92 B at config 5, whose bin key has 24 bits)."""
+    return n_tl * (44.0 + 16.0 * ((info["key_bits"] + 7) // 8))
+
+
+def load_bytes_model(info: dict, n_tl: int) -> float:
+    """What THIS implementation moves with the sort it used: not the roofline's numerator."""
     if info["sort_kind"] == 1:
         return n_tl * 128.0 + 20.0 * info["n_bins"]
     return n_tl * (76.0 + 20.0 * info["n_passes"])
@@ -315,11 +321,13 @@ def run_ours(args, spec, cfg):
     peak_tf = fp32_peak_tflops(props.multi_processor_count, peaks["sm_max_mhz"])
     if units is not None:
         flops = float(np.mean([sum(FLOP[k] * u[k] for k in FLOP) for u in units]))
-        cand = float(np.mean([u["n_cand"] for u in units]))
-        units_src = "tests/golden/units_timeframe.json (oracle counters per 500k-track launch)"
+        # distinct tracklets found inside some road, counted by the oracle (each read once: SURVEY.md 8(d).3)
+        cand = float(np.mean([u.get("n_distinct_cand", min(u["n_cand"], n_tl)) for u in units]))
+        units_src = "tests/golden/units_timeframe.json (oracle counters per 500k-track launch; n_distinct_cand for the bytes)"
     else:                                          # other workloads: count what the GPU itself reported
-        flops, cand, units_src = None, n_evals / nb, "n_cand from the kernel's own counter; flops not frozen for this workload"
-    bytes_alg = (BYTES_TRACK_IN + BYTES_TRACK_OUT) * (n / nb) + min(cand, n_tl) * BYTES_PER_CAND
+        flops, cand = None, min(n_evals / nb, n_tl)
+        units_src = "n_cand from the kernel's own counter (an upper bound of the distinct ones); flops not frozen for this workload"
+    bytes_alg = (BYTES_TRACK_IN + BYTES_TRACK_OUT) * (n / nb) + cand * BYTES_PER_CAND
     t_hbm = bytes_alg / (peaks["hbm_gbs"] * 1e9)
     t_alu = (flops / (peak_tf * 1e12)) if flops else 0.0
     if t_alu >= t_hbm:
@@ -328,6 +336,9 @@ def run_ours(args, spec, cfg):
     else:
         ach = bytes_alg / (match_avg_ms * 1e-3) / 1e9
         roof = dict(bound="hbm", achieved=ach, peak=peaks["hbm_gbs"], unit="GB/s", frac=ach / peaks["hbm_gbs"], traffic=None)
+    roof["bounds_ms"] = dict(t_alu=1e3 * t_alu, t_hbm=1e3 * t_hbm, binds="alu" if t_alu >= t_hbm else "hbm",
+                             note="roofline time per launch = the slower of algorithmic flops at the FP32 peak and algorithmic "
+                                  "bytes at the measured HBM bandwidth (SURVEY.md 8(d).3 constants)")
     roof["alu_view"] = dict(achieved_tflops=(flops / (match_avg_ms * 1e-3) / 1e12) if flops else None, peak_tflops=peak_tf)
     roof.update(kernel="match_kernel<4,BINNED>" if spec.n_hyp in (3, 4) else f"match_kernel (n_hyp={spec.n_hyp})",
                 launch_ms=match_avg_ms, trd_match_call_ms=match_call_ms,
@@ -336,12 +347,25 @@ def run_ours(args, spec, cfg):
                 roofline_ms_per_launch=1e3 * max(t_alu, t_hbm), hbm_view_gbs=bytes_alg / (match_avg_ms * 1e-3) / 1e9,
                 peak_source=f"HBM {peaks['source']} (MEASURED_PEAKS.json); FP32 = {props.multi_processor_count} SMs x 128 x 2 x "
                             f"{peaks['sm_max_mhz']:.0f} MHz", units=units_src,
-                load_tracklets_ms=load_ms, load_algorithmic_gbs=load_bytes(info, n_tl) / (load_ms * 1e-3) / 1e9,
-                load_io_gbs=n_tl * 32 / (load_ms * 1e-3) / 1e9)
+                load_tracklets_ms=load_ms,
+                load_algorithmic_gbs=load_bytes_algorithmic(info, n_tl) / (load_ms * 1e-3) / 1e9,
+                load_frac_of_hbm=load_bytes_algorithmic(info, n_tl) / (load_ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                load_model_gbs=load_bytes_model(info, n_tl) / (load_ms * 1e-3) / 1e9,
+                load_io_gbs=n_tl * 32 / (load_ms * 1e-3) / 1e9,
+                load_note="load_algorithmic_gbs: SURVEY.md 8(d).3 bytes (44 + 16 x passes per tracklet); load_model_gbs: the bytes "
+                          "this implementation's passes move (DESIGN.md 6.1); load_io_gbs: 16 B in + 16 B out per tracklet")
     prof = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(prof):
+    if os.path.exists(prof) and spec.name == "timeframe":
         with open(prof) as f:
-            roof["traffic"] = json.load(f).get("match_kernel_dram_bytes_per_launch")
+            tj = json.load(f)
+        roof["traffic"] = tj.get("match_kernel_dram_bytes_per_launch")
+        roof["traffic_source"] = "profiles/traffic.json (one ncu --set full capture of this kernel, NOT measured in this run): " + tj.get("source", "")
+        wi = tj.get("match_kernel_warp_instructions_per_launch")
+        if wi:
+            issue_ms = 1e3 * wi / (props.multi_processor_count * 4 * peaks["sm_max_mhz"] * 1e6)
+            roof["issue_view"] = dict(warp_instructions_per_launch=wi, issue_only_ms=issue_ms, frac_of_launch=issue_ms / match_avg_ms,
+                                      note="executed warp instructions (same ncu capture) / (SMs x 4 schedulers x max clock): the time "
+                                           "the kernel would take if it issued one instruction per scheduler and cycle")
 
     line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=max(args.warmup, 3),
                 ms_per_step=ms_per_step, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32",
@@ -366,12 +390,82 @@ def run_ours(args, spec, cfg):
         n_sample = min(ORACLE_SAMPLE_TRACKS, n)
         r, cores = oracle_sample(cfg, data, n_sample)
         full_s = r["seconds"]["index"] + r["seconds"]["match"] * n / n_sample
+        n_1t = min(ORACLE_SAMPLE_TRACKS_1T, n)
+        r1, _ = oracle_sample(cfg, data, n_1t, n_threads=1)
+        full_1t = r1["seconds"]["index"] + r1["seconds"]["match"] * n / n_1t
         line["cpu_baseline"] = dict(
-            value=n / full_s, unit=UNIT, cores=cores, kind="oracle",
+            value=n / full_s, unit=UNIT, cores=cores, kind="oracle (unoptimised: plain double-precision checker, its index is one "
+                                                            "y-sorted list per (sector, layer) without z binning)",
+            value_1t=n / full_1t,
+            scanned_per_in_road_candidate=r["counters"]["n_scanned"] / max(r["counters"]["n_cand"], 1),
             sample=(f"first {n_sample} of {n} tracks against all {n_tl} tracklets: index build {r['seconds']['index']:.2f} s + "
-                    f"match {r['seconds']['match']:.2f} s; value = n_tracks / (index + match x {n / n_sample:.0f})"))
+                    f"match {r['seconds']['match']:.2f} s; value = n_tracks / (index + match x {n / n_sample:.0f}); value_1t: the same "
+                    f"with one thread on the first {n_1t} tracks (index {r1['seconds']['index']:.2f} s + match {r1['seconds']['match']:.2f} s)"))
     print(json.dumps(line), flush=True)
     D.shutdown()
+
+
+def run_sweep(args):
+    """`--sweep`: the three curves of the paper's benchmark (Fig. 5: time per event against
+    the number of tracks for the CPU with one thread, the CPU with all cores and the GPU) on the five configs of
+    BASELINE.json.  GPU: one step = trd_load_tracklets + trd_match over all batches, device-resident, CUDA events.
+    CPU: the oracle as it stands (index build + matching), on a bounded sample for config 5.  One JSON line per config
+    and a markdown table at the end."""
+    import torch
+    from paper_2003_03174_b200 import binding as B, build as Bd, workloads as W
+    from oracle import oracle as O
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the TRD matcher has no CPU fallback")
+    Bd.build()
+    torch.cuda.set_device(0)
+    stream = torch.cuda.current_stream()
+    rows = []
+    for name in ("tiny", "central", "central8", "pileup", "timeframe"):
+        spec = W.CONFIGS[name]; data = W.generate(spec); cfg = W.matcher_config(spec)
+        n, n_tl = spec.n_tracks, int(data["tl_y"].shape[0])
+        batch = spec.batch or n
+        bounds = [(lo, min(n, lo + batch)) for lo in range(0, n, batch)]
+        dev = B.to_device(data, torch.device("cuda", 0))
+        tracks = [dict(par=dev["par"][:, lo:hi].contiguous(), cov=dev["cov"][:, lo:hi].contiguous(),
+                       x=dev["x"][lo:hi].contiguous(), sector=dev["sector"][lo:hi].contiguous()) for lo, hi in bounds]
+        outs = [B.alloc_tracks_out(hi - lo, torch.device("cuda", 0)) for lo, hi in bounds]
+        h = B.trd_create(cfg)
+
+        def step():
+            B.trd_load_tracklets(h, dev["tl_y"], dev["tl_z"], dev["tl_dydx"], dev["tl_chamber"], stream=stream)
+            for t, o in zip(tracks, outs):
+                B.trd_match(h, t, o, stream=stream)
+
+        steps = args.steps if name == "timeframe" else max(args.steps, 50)
+        for _ in range(5):
+            step()
+        torch.cuda.synchronize()
+        e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(steps):
+            step()
+        e1.record(stream); torch.cuda.synchronize()
+        gpu_ms = e0.elapsed_time(e1) / steps
+        B.trd_destroy(h)
+        n_all = min(ORACLE_SAMPLE_TRACKS, n); n_1t = min(ORACLE_SAMPLE_TRACKS_1T, n)
+        ra = O.match(cfg, data, lo=0, hi=n_all)
+        r1 = O.match(cfg, data, lo=0, hi=n_1t, n_threads=1)
+        cpu_all_ms = 1e3 * (ra["seconds"]["index"] + ra["seconds"]["match"] * n / n_all)
+        cpu_1t_ms = 1e3 * (r1["seconds"]["index"] + r1["seconds"]["match"] * n / n_1t)
+        row = dict(sweep=name, n_tracks=n, n_tracklets=n_tl, n_hyp=spec.n_hyp, n_sigma_road=spec.n_sigma_road,
+                   gpu_ms_per_step=gpu_ms, gpu_tracks_per_s=n / (gpu_ms * 1e-3), gpu_steps=steps,
+                   oracle_cores=O.max_threads(), oracle_all_cores_ms=cpu_all_ms, oracle_1_thread_ms=cpu_1t_ms,
+                   oracle_sample_tracks=[n_all, n_1t], unit="ms per step (load + match of the whole config)")
+        rows.append(row)
+        print(json.dumps(row), flush=True)
+        del dev, tracks, outs
+        torch.cuda.empty_cache()
+    print("\n| config | tracks | tracklets | nHyp | oracle, 1 thread | oracle, %d threads | GPU (B200) | GPU tracks/s |" % rows[0]["oracle_cores"])
+    print("|---|---|---|---|---|---|---|---|")
+    for r in rows:
+        print("| %s | %d | %d | %d | %.1f ms | %.1f ms | %.3f ms | %.3g |" % (
+            r["sweep"], r["n_tracks"], r["n_tracklets"], r["n_hyp"], r["oracle_1_thread_ms"], r["oracle_all_cores_ms"],
+            r["gpu_ms_per_step"], r["gpu_tracks_per_s"]))
 
 
 def main():
@@ -383,6 +477,7 @@ def main():
     ap.add_argument("--workload", default="timeframe")
     ap.add_argument("--tracks", type=int, default=0, help="scale the workload to this many tracks (debugging)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweep", action="store_true", help="configs 1-5: oracle with one thread, oracle with all cores, GPU (PAPER.md Fig. 5)")
     ap.add_argument("--interactions", type=int, default=0,
                     help="> 1: time-frame association with this many interactions (SURVEY.md 8(f) NEXT#2)")
     ap.add_argument("--ybin-width", type=float, default=0.0, help="local-y bin width of the index in cm (0 = chosen by the library)")
@@ -395,6 +490,9 @@ def main():
     ap.add_argument("--res-model", type=int, default=0, choices=[0, 1],
                     help="1: inputs and matcher with the sin(phi)-dependent resolutions and pad tilt (SURVEY.md 8(f) NEXT#1)")
     args = ap.parse_args()
+    if args.sweep:
+        run_sweep(args)
+        return
     from paper_2003_03174_b200 import workloads as W
     spec = W.CONFIGS[args.workload]
     if args.tracks:

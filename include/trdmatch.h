@@ -167,11 +167,15 @@ typedef struct trd_handle trd_handle;
 
 int trd_version(void);
 
-/* Validates and copies *cfg, derives the float32 constants.  Allocates nothing proportional
+/* The matcher for one geometry and one set of cuts: the 18 x 5 x 6 segmentation and layer planes of PAPER.md:50
+ * (section 3, second paragraph), the search road and the chi2 from y and z only of PAPER.md:52 (n_sigma_road, chi2_cut),
+ * the 4 sigma inclination veto and the N hypotheses kept per layer of PAPER.md:60 (n_sigma_angle, n_hyp).
+ * Validates and copies *cfg, derives the float32 constants.  Allocates nothing proportional
  * to data.  The library owns *out until trd_destroy. */
 int trd_create(const trd_config* cfg, trd_handle** out);
 
-/* Frees everything the handle owns (synchronises the device first).  NULL is a no-op. */
+/* Frees everything the handle owns (synchronises the device first).  NULL is a no-op.  (Housekeeping: no passage of
+ * the paper defines it.) */
 void trd_destroy(trd_handle* h);
 
 /* Builds the tracklet index on the device (north_star: "device-side sort and index by chamber
@@ -202,7 +206,11 @@ int trd_load_tracklets_tf(trd_handle* h, const float* d_y, const float* d_z, con
  * with the NEXT trd_load_tracklets (the loaded index is dropped). */
 int trd_set_chamber_dx(trd_handle* h, const float* dx, int32_t n_chambers, void* stream);
 
-/* The tracking step for one batch (n_tracks >= 0) against the loaded index. */
+/* The tracking step for one batch (n_tracks >= 0) against the loaded index -- PAPER.md:52-64 (section 3, paragraphs 3-5)
+ * and Fig. 2: every track is extrapolated to each TRD layer (L52, L64), the tracklets inside the search
+ * road derived from its covariance are its candidates (L52), those whose inclination is more than 4 sigma off are
+ * excluded (L60), chi2 is computed from y and z only (L52), the best n_hyp hypotheses per layer are kept (L60) and
+ * updated with a Kalman filter (L9, L40); tracks are independent (L86). */
 int trd_match(trd_handle* h, const trd_tracks_in* in, const trd_tracks_out* out, int64_t n_tracks,
               void* stream);
 
@@ -239,7 +247,8 @@ int trd_match_host(trd_handle* h, const trd_tracks_in* in_host, const trd_tracks
 int trd_get_index_info(const trd_handle* h, trd_index_info* info);
 int trd_copy_index(trd_handle* h, int32_t* sorted_pos, uint32_t* sorted_key, int32_t* bin_first, void* stream);
 const char* trd_last_error(const trd_handle* h);
-int64_t trd_device_bytes(const trd_handle* h);   /* device memory currently owned by the handle */
+int64_t trd_device_bytes(const trd_handle* h);   /* device memory currently owned by the handle (SURVEY.md 8(b) calls it
+                                                     trd_scratch_bytes; renamed because it also counts the sorted store) */
 int64_t trd_kernel_launches(const trd_handle* h); /* kernels launched through this handle so far */
 /* Device time of the match kernel alone in the most recent trd_match (CUDA events recorded on the call's
  * stream around that one launch; waits for the end event).  TRD_E_STATE if no trd_match has run. */

@@ -168,7 +168,7 @@ def candidates(cfg: dict, tl: dict, p, c15, sector: int, layer: int, brute: bool
 
 
 def match(cfg: dict, data: dict, brute: bool = False, n_threads: int = 0, lo: int = 0,
-          hi: Optional[int] = None) -> dict:
+          hi: Optional[int] = None, count_distinct: bool = False) -> dict:
     """The whole tracking step on tracks [lo, hi) of `data` against all its tracklets.
 
     `data` holds the float32 arrays of paper_2003_03174_b200.workloads.generate (or any dict with the
@@ -199,16 +199,20 @@ def match(cfg: dict, data: dict, brute: bool = False, n_threads: int = 0, lo: in
     if dx is not None:
         dx = np.ascontiguousarray(dx, np.float64)
         assert dx.shape[0] == cfg["n_sectors"] * cfg["n_stacks"] * cfg["n_layers"]
+    touched = np.zeros(y.shape[0], np.uint8) if count_distinct else None
     rc = lib().orc_match(C.byref(make_config(cfg)), _fp(y), _fp(z), _fp(d), _ip(ch), C.c_int64(y.shape[0]),
                          _fp(par), _fp(cov), _fp(x), _ip(sec), C.c_int64(n), int(brute), int(n_threads),
                          _ip(out["idx"]), _dp(out["par"]), _dp(out["cov"]), _dp(out["x"]), _ip(out["sector"]),
                          _dp(out["chi2"]), _ip(out["n_matched"]), _ip(out["n_evals"]), _dp(out["margin"]),
                          counters.ctypes.data_as(C.POINTER(C.c_int64)), _dp(seconds), *ia_args,
-                         _dp(dx) if dx is not None else None)
+                         _dp(dx) if dx is not None else None,
+                         touched.ctypes.data_as(C.POINTER(C.c_ubyte)) if touched is not None else None)
     if rc != 0:
         raise RuntimeError(f"orc_match failed: {rc}")
     out["counters"] = dict(zip(("n_prop", "n_rot", "n_road", "n_cand", "n_upd", "n_scanned"), counters.tolist()))
     out["seconds"] = dict(index=float(seconds[0]), match=float(seconds[1]))
+    if touched is not None:
+        out["counters"]["n_distinct_cand"] = int(touched.sum())     # distinct tracklets inside some road
     return out
 
 

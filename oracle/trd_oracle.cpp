@@ -87,6 +87,7 @@ struct Tracklet {
 
 struct Counters {
     int64_t n_prop = 0, n_rot = 0, n_road = 0, n_cand = 0, n_upd = 0, n_scanned = 0;
+    unsigned char* touched = nullptr;   // optional, one byte per tracklet: set for every tracklet found inside a road
 };
 
 // kappa = b q/pT; b from the field at the point (x, y, z) of the current sector frame (r^2 = x^2 + y^2 in any frame) [R35]
@@ -463,6 +464,7 @@ void find_candidates(const Config& cfg, const Store& st, const Hyp& h, int layer
         if (!(in_y && in_z && pass)) continue;
         if (n_evals) (*n_evals)++;                                          // one "candidate evaluation"
         if (cnt) cnt->n_cand++;
+        if (cnt && cnt->touched) cnt->touched[tl.index] = 1;              // distinct in-road tracklets (roofline bytes)
         if (cut) continue;
         out.push_back({tl.index, tl.y, tl.z, c2, tl.dx});
     }
@@ -686,13 +688,15 @@ int orc_candidates(const orc_config* cfg, const float* y, const float* z, const 
 // par: 5 x n_trk, cov: 15 x n_trk (SoA, row = component).  Outputs are double / int32 SoA:
 // out_idx 6 x n_trk, out_par 5 x n_trk, out_cov 15 x n_trk.  brute != 0 ignores the sorted
 // index and loops over all tracklets of the (sector, layer).  counters: n_prop, n_rot,
-// n_road, n_cand, n_upd, n_scanned.  seconds: index build, matching.
+// n_road, n_cand, n_upd, n_scanned.  seconds: index build, matching.  out_touched (optional, n_tl bytes, zeroed by the
+// caller): set to 1 for every tracklet that was inside the road of some hypothesis of some track.
 int orc_match(const orc_config* cfg, const float* tl_y, const float* tl_z, const float* tl_dydx,
               const int32_t* tl_chamber, int64_t n_tl, const float* par, const float* cov, const float* x,
               const int32_t* sector, int64_t n_trk, int brute, int n_threads, int32_t* out_idx, double* out_par,
               double* out_cov, double* out_x, int32_t* out_sector, double* out_chi2, int32_t* out_n_matched,
               int32_t* out_n_evals, double* out_margin, int64_t counters[6], double seconds[2],
-              const int32_t* tl_ia, const int32_t* trk_ia, int32_t n_ia, const double* chamber_dx) {
+              const int32_t* tl_ia, const int32_t* trk_ia, int32_t n_ia, const double* chamber_dx,
+              unsigned char* out_touched) {
     if (cfg->n_layers > kMaxLayers || cfg->n_hyp < 1) return -1;
     if ((tl_ia == nullptr) != (trk_ia == nullptr)) return -2;
     const auto t0 = std::chrono::steady_clock::now();
@@ -706,6 +710,7 @@ int orc_match(const orc_config* cfg, const float* tl_y, const float* tl_z, const
 #pragma omp parallel
     {
         Counters local;
+        local.touched = out_touched;                  // every thread only ever stores 1: no race that matters
 #pragma omp for schedule(dynamic, 256)
         for (int64_t i = 0; i < n_trk; ++i) {
             double p[5], c15[15];

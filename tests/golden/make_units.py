@@ -1,5 +1,5 @@
 """Writes tests/golden/units_timeframe.json: the oracle's operation counters (n_prop, n_rot, n_road, n_cand,
-n_upd) for each 500k-track batch of BASELINE.json configs[4] ("timeframe", seed 317405), i.e. the number of
+n_upd, and n_distinct_cand = distinct tracklets found inside some road) for each 500k-track batch of BASELINE.json configs[4] ("timeframe", seed 317405), i.e. the number of
 algorithmic units one trd_match launch of bench.py processes.
 Calls only oracle/ and the seeded input generator -- never the CUDA path.  Takes a few minutes of CPU.
     python tests/golden/make_units.py
@@ -20,7 +20,7 @@ def main():
     cfg = W.matcher_config(spec)
     batches = []
     for lo in range(0, spec.n_tracks, spec.batch):
-        r = O.match(cfg, d, lo=lo, hi=lo + spec.batch)
+        r = O.match(cfg, d, lo=lo, hi=lo + spec.batch, count_distinct=True)
         c = dict(r["counters"]); c["n_tracks"] = spec.batch
         c["n_matched_ge2"] = int((r["n_matched"] >= 2).sum())
         c["n_fragile_1e-4"] = int((r["margin"] < 1e-4).sum())
