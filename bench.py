@@ -129,13 +129,14 @@ def load_bytes_model(info: dict, n_tl: int) -> float:
     return n_tl * (76.0 + 20.0 * info["n_passes"])
 
 
-def config_dict(spec, n_tl, world):
+def config_dict(spec, n_tl, world, strong=False):
     n, batch = spec.n_tracks, spec.batch or spec.n_tracks
     nb = (n + batch - 1) // batch
     return dict(workload=spec.name, n_tracks=n, n_tracklets=n_tl, n_hyp=spec.n_hyp, n_sigma_road=spec.n_sigma_road,
                 batch=batch, step="1 trd_load_tracklets + %d trd_match" % nb,
                 l2="inputs larger than L2 (%.0f MB tracklets + %.0f MB tracks per step)" % (16e-6 * n_tl, 88e-6 * n),
-                parallelism=f"{world} x independent time frames, no collective")
+                parallelism=(f"1 time frame, tracks split over {world} ranks, index replicated, no collective" if strong else
+                             f"{world} x independent time frames, no collective"))
 
 
 def oracle_sample(cfg, data, n_sample, n_threads=0):
@@ -191,7 +192,14 @@ def run_ours(args, spec, cfg):
     data = W.generate(spec)                     # every rank: its own (identically generated) time frame
     n, n_tl = spec.n_tracks, int(data["tl_y"].shape[0])
     batch = spec.batch or n
-    bounds = [(lo, min(n, lo + batch)) for lo in range(0, n, batch)]
+    strong = args.scaling == "strong" and world > 1
+    if strong:
+        # ONE frame split over the ranks: contiguous track slices, the index built on every rank
+        # (replicated: 0.3 GB against 180 GB of HBM), outputs left sharded, still no data-path collective
+        s_lo, s_hi = D.track_slice(n, rank, world)
+        bounds = [(lo, min(s_hi, lo + batch)) for lo in range(s_lo, s_hi, batch)]
+    else:
+        bounds = [(lo, min(n, lo + batch)) for lo in range(0, n, batch)]
     dev = B.to_device(data, device)
     tracks = [dict(par=dev["par"][:, lo:hi].contiguous(), cov=dev["cov"][:, lo:hi].contiguous(),
                    x=dev["x"][lo:hi].contiguous(), sector=dev["sector"][lo:hi].contiguous()) for lo, hi in bounds]
@@ -252,12 +260,16 @@ def run_ours(args, spec, cfg):
     n_refitted = int(sum(int((ro["n_used"] >= 2).sum().item()) for ro in r_outs))
     total_ms = D.max_over_ranks(t_start.elapsed_time(t_end), device)
     ms_per_step = total_ms / args.steps
-    value = world * n / (ms_per_step * 1e-3)
+    n_job = n if strong else world * n            # tracks the whole job matched per step
+    value = n_job / (ms_per_step * 1e-3)
     nb = len(bounds)
     load_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in events]))
     match_ms = np.array([[e[1 + k].elapsed_time(e[2 + k]) for k in range(nb)] for e in events])   # steps x batches
     n_evals = int(sum(int(o["n_evals"].sum().item()) for o in outs))
     n_ge2 = int(sum(int((o["n_matched"] >= 2).sum().item()) for o in outs))
+    n_mine = sum(hi - lo for lo, hi in bounds)       # tracks this rank matched per step
+    if strong:
+        n_evals = int(D.sum_over_ranks(n_evals, device))
 
     e2e_s, e2e_steps = None, 0
     if n_ia <= 1:
@@ -303,8 +315,8 @@ def run_ours(args, spec, cfg):
         D.barrier()
         for o, ho in zip(outs, h_outs):               # the two entry points must agree bit for bit
             assert np.array_equal(o["idx"].cpu().numpy(), ho["idx"]) and np.array_equal(o["chi2"].cpu().numpy(), ho["chi2"])
-    h2d = 16 * n_tl + BYTES_TRACK_IN * n
-    d2h = BYTES_TRACK_OUT * n
+    h2d = 16 * n_tl + BYTES_TRACK_IN * n_mine
+    d2h = BYTES_TRACK_OUT * n_mine
     info = B.trd_get_index_info(h)
     B.trd_destroy(h)
 
@@ -327,7 +339,7 @@ def run_ours(args, spec, cfg):
     else:                                          # other workloads: count what the GPU itself reported
         flops, cand = None, min(n_evals / nb, n_tl)
         units_src = "n_cand from the kernel's own counter (an upper bound of the distinct ones); flops not frozen for this workload"
-    bytes_alg = (BYTES_TRACK_IN + BYTES_TRACK_OUT) * (n / nb) + cand * BYTES_PER_CAND
+    bytes_alg = (BYTES_TRACK_IN + BYTES_TRACK_OUT) * (n_mine / nb) + cand * BYTES_PER_CAND
     t_hbm = bytes_alg / (peaks["hbm_gbs"] * 1e9)
     t_alu = (flops / (peak_tf * 1e12)) if flops else 0.0
     if t_alu >= t_hbm:
@@ -368,18 +380,19 @@ def run_ours(args, spec, cfg):
                                            "the kernel would take if it issued one instruction per scheduler and cycle")
 
     line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=max(args.warmup, 3),
-                ms_per_step=ms_per_step, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32",
+                ms_per_step=ms_per_step, higher_is_better=True, scaling="strong" if strong else "weak", vs_baseline=None,
+                dtype="f32 (y, sin(phi) accumulated in f64)",
                 data="synthetic",
-                config=config_dict(spec, n_tl, world),
-                cand_evals_per_s=world * n_evals / (ms_per_step * 1e-3), n_cand_evals=n_evals,
-                frac_tracks_ge2_tracklets=n_ge2 / n, index=dict(n_ybins=info["n_ybins"], n_zrows=info["n_zrows"],
+                config=config_dict(spec, n_tl, world, strong),
+                cand_evals_per_s=(1 if strong else world) * n_evals / (ms_per_step * 1e-3), n_cand_evals=n_evals,
+                frac_tracks_ge2_tracklets=n_ge2 / max(n_mine, 1), index=dict(n_ybins=info["n_ybins"], n_zrows=info["n_zrows"],
                                                                 ybin_width_cm=info["ybin_width"],
                                                                 sort="counting" if info["sort_kind"] == 1 else "radix",
                                                                 radix_passes=0 if info["sort_kind"] == 1 else info["n_passes"]),
-                refit=dict(ms_per_time_frame=refit_ms, tracks_per_s=n / (refit_ms * 1e-3), frac_refitted=n_refitted / n,
+                refit=dict(ms_per_time_frame=refit_ms, tracks_per_s=n_mine / (refit_ms * 1e-3), frac_refitted=n_refitted / max(n_mine, 1),
                            note="trd_refit over the matched chains of the step, device-resident, timed separately"),
                 clocks=clocks, gpu_launches=int(launches),
-                e2e=(dict(value=world * n / e2e_s, unit=UNIT, h2d_bytes_per_step=int(h2d), d2h_bytes_per_step=int(d2h),
+                e2e=(dict(value=n_job / e2e_s, unit=UNIT, h2d_bytes_per_step=int(h2d), d2h_bytes_per_step=int(d2h),
                           ms_per_step=1e3 * e2e_s, steps=e2e_steps, ms_per_step_frame_by_frame=1e3 * e2e_sync_s,
                           note="consecutive frames streamed through the host entry points (copies of frame k+1 overlap the "
                                "kernels of frame k); frame_by_frame waits for each frame's results before the next") if e2e_s else
@@ -475,6 +488,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="timeframe")
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="N > 1: weak = one time frame per rank (default); strong = one frame, its tracks split over the ranks")
     ap.add_argument("--tracks", type=int, default=0, help="scale the workload to this many tracks (debugging)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", action="store_true", help="configs 1-5: oracle with one thread, oracle with all cores, GPU (PAPER.md Fig. 5)")

@@ -65,3 +65,17 @@ def max_over_ranks(value: float, device="cpu") -> float:
 
 def sum_over_ranks(value: float, device="cpu") -> float:
     return _reduce(value, "SUM", device)
+
+
+def gather_sharded(shard: dict, n_tracks: int) -> dict:
+    """Strong scaling leaves the outputs sharded by `track_slice`; this puts the shards of all ranks back together
+    (last axis = tracks, rank order = track order) on every rank.  Not part of any timed path."""
+    import numpy as np
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return shard
+    parts = [None] * dist.get_world_size()
+    dist.all_gather_object(parts, {k: np.ascontiguousarray(v) for k, v in shard.items()})
+    full = {k: np.concatenate([p[k] for p in parts], axis=-1) for k in shard}
+    assert all(v.shape[-1] == n_tracks for v in full.values())
+    return full

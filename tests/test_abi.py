@@ -82,10 +82,7 @@ def test_product_path_does_not_reach_the_oracle():
                 assert "from oracle" not in text and "import oracle" not in text and "trd_oracle" not in text, f
 
 
-def test_plain_c_program_links_and_calls_the_library(lib):
-    """A C99 program (no Python, no torch) links against libtrdmatch.so and uses the ABI: version, argument
-    errors, and -- on a machine without a GPU -- the loud TRD_E_CUDA from trd_create."""
-    src = r'''
+C_PROGRAM = r'''
 #include "trdmatch.h"
 #include <stdio.h>
 #include <string.h>
@@ -100,18 +97,65 @@ int main(void) {
     { double x[6] = {300, 313, 326, 338, 351, 364}; memcpy(c.layer_x, x, sizeof x); }
     c.z_max = 350; c.pad_length = 8; c.bz_tesla = 0.5; c.sigma_y = 0.04; c.sigma_z = 2.3094; c.sigma_dydx = 0.02;
     c.n_sigma_road = 3; c.n_sigma_angle = 4; c.chi2_cut = 15; c.chi2_penalty = 15; c.max_snp = 0.95;
-    { int rc = trd_create(&c, &h); printf("%d\n", rc); if (rc == TRD_OK) { trd_destroy(h); } else if (rc != TRD_E_CUDA) return 4; }
+    { int rc = trd_create(&c, &h); printf("%d\n", rc); if (rc == TRD_E_CUDA) { trd_destroy(0); return 0; } if (rc != TRD_OK) return 4; }
+    {   /* two infinite-momentum tracks (q/pT = 0) along x: track 0 in sector 4 at y = 1, z = 4; track 1 in sector 9 at
+           y = -2, z = -12 with no tracklet in layer 3.  Tracklets sit exactly on the lines, z on pad-row centres. */
+        float ty[12], tz[12], td[12]; int32_t tc[12]; int n = 0, l, k;
+        float par[5][2] = {{1.0f, -2.0f}, {4.0f, -12.0f}, {0.0f, 0.0f}, {0.0f, 0.0f}, {0.0f, 0.0f}};
+        float cov[15][2]; float x[2] = {247.0f, 247.0f}; int32_t sec[2] = {4, 9};
+        float opar[5][2], ocov[15][2], ox[2], ochi2[2]; int32_t oidx[TRD_MAX_LAYERS][2], osec[2], onm[2], oev[2];
+        trd_tracks_in in; trd_tracks_out out;
+        for (l = 0; l < 6; ++l) { ty[n] = 1.0f; tz[n] = 4.0f; td[n] = 0.0f; tc[n] = 4 * 30 + 2 * 6 + l; ++n; }
+        for (l = 0; l < 6; ++l) { if (l == 3) continue; ty[n] = -2.0f; tz[n] = -12.0f; td[n] = 0.0f; tc[n] = 9 * 30 + 2 * 6 + l; ++n; }
+        ty[n] = 1.0f; tz[n] = 4.0f; td[n] = 0.0f; tc[n] = 5 * 30 + 2 * 6 + 2; ++n;       /* same place, other sector: never a candidate */
+        memset(cov, 0, sizeof cov);
+        for (k = 0; k < 2; ++k) { cov[0][k] = 0.01f; cov[2][k] = 0.01f; cov[5][k] = 1e-6f; cov[9][k] = 1e-6f; cov[14][k] = 1e-4f; }
+        memset(&in, 0, sizeof in); memset(&out, 0, sizeof out);
+        for (k = 0; k < 5; ++k) { in.par[k] = par[k]; out.par[k] = opar[k]; }
+        for (k = 0; k < 15; ++k) { in.cov[k] = cov[k]; out.cov[k] = ocov[k]; }
+        in.x = x; in.sector = sec;
+        for (l = 0; l < TRD_MAX_LAYERS; ++l) out.tracklet_idx[l] = oidx[l];
+        out.x = ox; out.sector = osec; out.chi2 = ochi2; out.n_matched = onm; out.n_cand_evals = oev;
+        if (trd_load_tracklets_host(h, ty, tz, td, tc, n, 0) != TRD_OK) { printf("%s\n", trd_last_error(h)); return 5; }
+        if (trd_match_host(h, &in, &out, 2, 0) != TRD_OK) { printf("%s\n", trd_last_error(h)); return 6; }
+        for (l = 0; l < 6; ++l) if (oidx[l][0] != l) return 7;
+        for (l = 0; l < 6; ++l) if (oidx[l][1] != (l == 3 ? -1 : (l < 3 ? 6 + l : 5 + l))) return 8;
+        if (onm[0] != 6 || onm[1] != 5 || osec[0] != 4 || osec[1] != 9 || ox[0] != 364.0f) return 9;
+        if (!(ochi2[0] >= 0.0f && ochi2[0] < 1e-6f) || opar[0][0] != 1.0f || opar[1][1] != -12.0f) return 10;
+        if (oev[0] != 6 || oev[1] != 5 || trd_kernel_launches(h) < 2) return 11;
+    }
+    trd_destroy(h);
     trd_destroy(0);
     return 0;
 }
 '''
+
+
+def _run_c_program():
     with tempfile.TemporaryDirectory() as td:
         cfile = os.path.join(td, "t.c"); exe = os.path.join(td, "t")
-        open(cfile, "w").write(src)
+        open(cfile, "w").write(C_PROGRAM)
         libdir = os.path.dirname(Bd.LIB_PATH)
         subprocess.check_call(["gcc", "-std=c99", "-Wall", "-Werror", "-I", os.path.join(ROOT, "include"), cfile, "-o", exe,
                                "-L", libdir, "-ltrdmatch", "-Wl,-rpath," + libdir])
-        out = subprocess.run([exe], capture_output=True, text=True)
+        return subprocess.run([exe], capture_output=True, text=True)
+
+
+def test_plain_c_program_links_and_calls_the_library(lib):
+    """A C99 program (no Python, no torch) links against libtrdmatch.so and uses the ABI: version, argument
+    errors, and -- on a machine without a GPU -- the loud TRD_E_CUDA from trd_create.  With a GPU it runs the whole
+    path through C: trd_load_tracklets_host + trd_match_host on two straight tracks and twelve tracklets placed on
+    their lines (one of them in a neighbouring sector, one layer left out), and checks the chains that come back."""
+    out = _run_c_program()
     assert out.returncode == 0, (out.returncode, out.stdout, out.stderr)
     import torch
     assert int(out.stdout.split()[0]) == (B.TRD_OK if torch.cuda.is_available() else B.TRD_E_CUDA)
+
+
+@pytest.mark.gpu
+def test_plain_c_program_runs_load_and_match_on_the_gpu(lib):
+    """The same C program on the GPU box: trd_create succeeds, so it goes on to trd_load_tracklets_host and
+    trd_match_host and checks the chains itself (exit code 0 only if they are right)."""
+    out = _run_c_program()
+    assert out.returncode == 0, (out.returncode, out.stdout, out.stderr)
+    assert int(out.stdout.split()[0]) == B.TRD_OK

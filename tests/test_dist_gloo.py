@@ -1,13 +1,17 @@
 """The N > 1 plumbing on CPU (gloo, world_size 2): track slices tile the time frame, the timing reduction is
-a max over ranks, counts add up.  The tracking step itself has no collective."""
+a max over ranks, counts add up, and the sharded outputs of a strong-scaling run put back together are the
+single-rank result (checked with the parity comparator).  The tracking step itself has no collective (DESIGN.md
+"Multi-GPU")."""
 import os
 import socket
+
+import numpy as np
 
 import pytest
 import torch
 import torch.multiprocessing as mp
 
-from paper_2003_03174_b200 import dist as D
+from paper_2003_03174_b200 import dist as D, parity as P
 
 
 def test_track_slices_tile_the_frame():
@@ -29,8 +33,22 @@ def _worker(rank, world, port, q):
     D.barrier()
     ms = D.max_over_ranks(10.0 + 5.0 * rank)           # the slower rank defines the step time
     total = D.sum_over_ranks(hi - lo)
-    q.put((rank, ms, total))
+    # strong scaling: every rank holds the results of its own slice of ONE frame; together they are the frame's
+    full = _fake_result(1001)
+    mine = {k: v[..., lo:hi] for k, v in full.items()}
+    back = D.gather_sharded(mine, 1001)
+    rep = P.compare(back, dict(full, margin=np.full(1001, np.inf)))
+    ok = rep["ok"] and rep["n_assign_mismatch"] == 0 and all(np.array_equal(back[k], full[k]) for k in full)
+    q.put((rank, ms, total, bool(ok)))
     D.shutdown()
+
+
+def _fake_result(n):
+    """A result-shaped dict from a fixed seed (the comparator holds none of the method's arithmetic)."""
+    rng = np.random.default_rng(7)
+    return dict(idx=rng.integers(-1, 1000, (6, n)).astype(np.int32), par=rng.normal(size=(5, n)), cov=np.abs(rng.normal(size=(15, n))),
+                x=np.full(n, 364.0), sector=rng.integers(0, 18, n).astype(np.int32), chi2=np.abs(rng.normal(size=n)),
+                n_matched=rng.integers(0, 7, n).astype(np.int32))
 
 
 def test_two_ranks_gloo():
@@ -44,4 +62,4 @@ def test_two_ranks_gloo():
     for p in procs:
         p.join(timeout=60)
         assert p.exitcode == 0
-    assert res == [(0, 15.0, 1001.0), (1, 15.0, 1001.0)]
+    assert res == [(0, 15.0, 1001.0, True), (1, 15.0, 1001.0, True)]
