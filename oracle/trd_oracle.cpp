@@ -566,7 +566,19 @@ void match_track(const Config& cfg, const Store& st, const Hyp& seed, TrackResul
         }
         hyps.swap(next);
     }
-    res.best = hyps[0];
+    // With displaced chambers the scores of the kept children were replaced by the exact ones AFTER the ranking [R30],
+    // so the list is no longer ordered by them: the output is the hypothesis with the lowest final score (the first of
+    // equals).  Without offsets this is hyps[0] and the gap was already recorded at the last layer.
+    size_t ib = 0;
+    if (st.dx_max > 0.0 && hyps.size() > 1) {
+        size_t i2 = 1;
+        for (size_t k = 1; k < hyps.size(); ++k) {
+            if (hyps[k].score < hyps[ib].score) { i2 = ib; ib = k; }
+            else if (i2 == ib || hyps[k].score < hyps[i2].score) i2 = k;
+        }
+        if (rank_gap(mg, hyps[ib].score, hyps[i2].score)) ib = i2;
+    }
+    res.best = hyps[ib];
 }
 
 inline int tri(int i, int j) { return i * (i + 1) / 2 + j; }

@@ -152,6 +152,7 @@ int trd_create(const trd_config* cfg, trd_handle** out) {
 
 void trd_destroy(trd_handle* h) {
     if (!h) return;
+    const trd::DeviceGuard on_device(h);
     cudaDeviceSynchronize();
     release(h->store);
     release(h->packed);
@@ -187,6 +188,7 @@ void trd_destroy(trd_handle* h) {
 int trd_load_tracklets(trd_handle* h, const float* d_y, const float* d_z, const float* d_dydx,
                        const int32_t* d_chamber, int64_t n, void* stream) {
     if (!h) return TRD_E_ARG;
+    const trd::DeviceGuard on_device(h);
     if (n < 0 || n >= (1 << 29) - 1) return fail(h, TRD_E_ARG, "trd_load_tracklets: n out of range (must be < 2^29 - 1)");
     if (n > 0 && (!d_y || !d_z || !d_dydx || !d_chamber)) return fail(h, TRD_E_ARG, "trd_load_tracklets: NULL array");
     const cudaError_t e = trd::build_index(h, d_y, d_z, d_dydx, d_chamber, nullptr, 1, n, (cudaStream_t)stream);
@@ -198,6 +200,7 @@ int trd_load_tracklets_tf(trd_handle* h, const float* d_y, const float* d_z, con
                           const int32_t* d_chamber, const int32_t* d_interaction, int32_t n_interactions, int64_t n,
                           void* stream) {
     if (!h) return TRD_E_ARG;
+    const trd::DeviceGuard on_device(h);
     if (n < 0 || n >= (1 << 29) - 1) return fail(h, TRD_E_ARG, "trd_load_tracklets_tf: n out of range (must be < 2^29 - 1)");
     if (n > 0 && (!d_y || !d_z || !d_dydx || !d_chamber)) return fail(h, TRD_E_ARG, "trd_load_tracklets_tf: NULL array");
     if (n_interactions > (1 << 20)) return fail(h, TRD_E_ARG, "trd_load_tracklets_tf: too many interactions");
@@ -209,6 +212,7 @@ int trd_load_tracklets_tf(trd_handle* h, const float* d_y, const float* d_z, con
 
 int trd_set_chamber_dx(trd_handle* h, const float* dx, int32_t n_chambers, void* stream) {
     if (!h) return TRD_E_ARG;
+    const trd::DeviceGuard on_device(h);
     cudaStream_t st = (cudaStream_t)stream;
     if (!dx || n_chambers == 0) {                        // back to the nominal planes
         h->mp.dx_max = 0.0f;
@@ -232,6 +236,7 @@ int trd_set_chamber_dx(trd_handle* h, const float* dx, int32_t n_chambers, void*
 
 int trd_refit(trd_handle* h, const trd_tracks_out* m, const trd_refit_out* out, int64_t n, void* stream) {
     if (!h) return TRD_E_ARG;
+    const trd::DeviceGuard on_device(h);
     if (!m || !out || n < 0) return fail(h, TRD_E_ARG, "trd_refit: NULL struct or negative n_tracks");
     if (!h->index_loaded) return fail(h, TRD_E_STATE, "trd_refit: no tracklets loaded");
     if (!(h->cfg.x_ref > 0.0)) return fail(h, TRD_E_ARG, "trd_refit: trd_config.x_ref must be positive");
@@ -253,6 +258,7 @@ int trd_refit(trd_handle* h, const trd_tracks_out* m, const trd_refit_out* out, 
 
 int trd_match(trd_handle* h, const trd_tracks_in* in, const trd_tracks_out* out, int64_t n_tracks, void* stream) {
     if (!h) return TRD_E_ARG;
+    const trd::DeviceGuard on_device(h);
     if (!in || !out || n_tracks < 0) return fail(h, TRD_E_ARG, "trd_match: NULL struct or negative n_tracks");
     if (!h->index_loaded) return fail(h, TRD_E_STATE, "trd_match: no tracklets loaded");
     if (n_tracks == 0) return TRD_OK;
@@ -288,6 +294,7 @@ int trd_get_index_info(const trd_handle* h, trd_index_info* info) {
 
 int trd_copy_index(trd_handle* h, int32_t* sorted_pos, uint32_t* sorted_key, int32_t* bin_first, void* stream) {
     if (!h) return TRD_E_ARG;
+    const trd::DeviceGuard on_device(h);
     if (!h->index_loaded) return fail(h, TRD_E_STATE, "trd_copy_index: no tracklets loaded");
     cudaStream_t st = (cudaStream_t)stream;
     cudaError_t e = cudaStreamSynchronize(st);
@@ -317,6 +324,7 @@ int64_t trd_kernel_launches(const trd_handle* h) { return h ? h->launches : 0; }
 
 int trd_match_kernel_ms(trd_handle* h, float* ms, int32_t n) {
     if (!h || !ms || n < 1) return TRD_E_ARG;
+    const trd::DeviceGuard on_device(h);
     if (n > trd_handle::kEvRing || n > h->ev_count) return fail(h, TRD_E_STATE, "trd_match_kernel_ms: fewer trd_match calls on record");
     for (int k = 0; k < n; ++k) {                     // ms[n - 1] is the most recent call
         cudaEvent_t* ev = h->ev_match[(h->ev_count - n + k) % trd_handle::kEvRing];

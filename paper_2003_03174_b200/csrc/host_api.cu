@@ -145,6 +145,7 @@ extern "C" {
 int trd_load_tracklets_host(trd_handle* h, const float* y, const float* z, const float* dydx,
                             const int32_t* chamber, int64_t n, void* stream) {
     if (!h) return TRD_E_ARG;
+    const trd::DeviceGuard on_device(h);
     if (n < 0 || n >= (1 << 29) - 1) return trd::fail(h, TRD_E_ARG, "trd_load_tracklets_host: n out of range (must be < 2^29 - 1)");
     if (n > 0 && (!y || !z || !dydx || !chamber)) return trd::fail(h, TRD_E_ARG, "trd_load_tracklets_host: NULL array");
     const cudaError_t e = trd::load_host(h, y, z, dydx, chamber, n, (cudaStream_t)stream);
@@ -154,6 +155,7 @@ int trd_load_tracklets_host(trd_handle* h, const float* y, const float* z, const
 
 int trd_match_host_async(trd_handle* h, const trd_tracks_in* in, const trd_tracks_out* out, int64_t n, void* stream) {
     if (!h) return TRD_E_ARG;
+    const trd::DeviceGuard on_device(h);
     if (!in || !out || n < 0) return trd::fail(h, TRD_E_ARG, "trd_match_host: NULL struct or negative n_tracks");
     if (!h->index_loaded) return trd::fail(h, TRD_E_STATE, "trd_match_host: no tracklets loaded");
     if (h->mp.g.n_ia > 1) return trd::fail(h, TRD_E_STATE, "trd_match_host: the index carries interactions; use trd_match");
@@ -173,6 +175,7 @@ int trd_match_host_async(trd_handle* h, const trd_tracks_in* in, const trd_track
 
 int trd_wait_host(trd_handle* h, void* stream) {
     if (!h) return TRD_E_ARG;
+    const trd::DeviceGuard on_device(h);
     const cudaError_t e = trd::wait_host(h, (cudaStream_t)stream);
     if (e != cudaSuccess) return trd::fail_cuda(h, e, "trd_wait_host");
     return TRD_OK;

@@ -168,6 +168,21 @@ cudaError_t place_tracks_by_key(trd_handle* h, const uint32_t* key, uint32_t* hi
                                 cudaStream_t stream);
 cudaError_t unpack_tracks(trd_handle* h, const float* rec_out, const trd_tracks_out& out, int64_t n, cudaStream_t stream);
 
+// Every entry point works on the device the handle was created on, whatever device is current in the calling thread:
+// the guard switches to it and restores the caller's device on the way out.
+struct DeviceGuard {
+    int prev = -1;
+    bool switched = false;
+    explicit DeviceGuard(const trd_handle* h) {
+        if (h && cudaGetDevice(&prev) == cudaSuccess && prev != h->device) switched = cudaSetDevice(h->device) == cudaSuccess;
+    }
+    ~DeviceGuard() {
+        if (switched) cudaSetDevice(prev);
+    }
+    DeviceGuard(const DeviceGuard&) = delete;
+    DeviceGuard& operator=(const DeviceGuard&) = delete;
+};
+
 int fail(trd_handle* h, int code, const std::string& what);
 int fail_cuda(trd_handle* h, cudaError_t e, const char* where);
 void host_pipeline_destroy(trd_handle* h);

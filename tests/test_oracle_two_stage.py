@@ -103,3 +103,63 @@ def test_sorted_index_equals_brute_force_with_offsets():
     a = O.match(cfg, d); b = O.match(cfg, d, brute=True)
     for k in KEYS:
         np.testing.assert_array_equal(a[k], b[k])
+
+
+def enumerate_chains_two_stage(cfg, d, i):
+    """Depth-first enumeration of ALL chains of track i with displaced chambers: at each layer every candidate the
+    linear extrapolation accepts (R29) -- attached after the EXACT propagation to its chamber's radius, scored with the
+    exact chi2 (R30) -- or skip.  Returns the sorted list of (exact score, idx tuple)."""
+    out = []
+    dx_ch = d["chamber_dx"].astype(np.float64)
+
+    def rec(L, p, c15, x, sec, alive, score, idx):
+        if L == 6:
+            out.append((score, tuple(idx)))
+            return
+        if alive:
+            ok, p2, c2, x2, sec2 = O.propagate_to_layer(cfg, p, c15, x, sec, cfg["layer_x"][L])
+            if ok:
+                p, c15, x, sec = p2, c2, x2, sec2
+                ci, _ = O.candidates(cfg, d, p, c15, sec, L, brute=True, chamber_dx=dx_ch)
+                for k in ci.tolist():
+                    dxk = dx_ch[d["tl_chamber"][k]]
+                    pe, ce, xe, ok2 = p, c15, x, True
+                    if dxk != 0.0:
+                        ok2, pe, ce, xe = O.propagate(cfg, p, c15, x, x + dxk)
+                    if not ok2:                                  # cannot get there: keeps its state, only skips from now on
+                        rec(L + 1, p, c15, x, sec, False, score, idx + [-1])
+                        continue
+                    pn, cn, inc = O.update(cfg, pe, ce, float(d["tl_y"][k]), float(d["tl_z"][k]), layer=L)
+                    rec(L + 1, pn, cn, xe, sec, abs(pn[2]) < cfg["max_snp"], score + inc, idx + [int(k)])
+            else:
+                alive = False
+        rec(L + 1, p, c15, x, sec, alive, score + cfg["chi2_penalty"], idx + [-1])
+
+    rec(0, d["par"][:, i].astype(float), d["cov"][:, i].astype(float), float(d["x"][i]), int(d["sector"][i]),
+        abs(float(d["par"][2, i])) < cfg["max_snp"], 0.0, [])
+    out.sort()
+    return out
+
+
+def test_output_is_the_chain_with_the_lowest_exact_score():
+    """With every child kept (nHyp = 4096) the matcher is exhaustive, and its output must be the chain with the lowest
+    EXACT total score -- the scores of the kept children are replaced by the exact chi2 after the ranking (R30), so the
+    first hypothesis of the list is not always the best one; the output is the minimum over the final list."""
+    # offsets of 2 cm and a soft spectrum: the linear extrapolation then differs from the exact step by the sagitta
+    # kappa dx^2 / 2 ~ 0.01-0.05 cm, of the order of the tracklet resolution, so the two rankings do disagree
+    spec = dataclasses.replace(W.CONFIGS["tiny"], name="dense_dx", number=31, n_tracks=60, n_noise=60000, n_hyp=4,
+                               chamber_dx_sigma=2.0, pt_spectrum="exp")
+    d = W.generate(spec); cfg = W.matcher_config(spec)
+    big = O.match(dict(cfg, n_hyp=4096), d)
+    n_multi = n_reordered = 0
+    for i in range(spec.n_tracks):
+        chains = enumerate_chains_two_stage(cfg, d, i)
+        assert len(chains) <= 4096
+        n_multi += len(chains) > 4
+        best_score, best_idx = chains[0]
+        if len(chains) > 1 and chains[1][0] - best_score < 1e-9 * max(best_score, 1.0):
+            continue                                             # an exact tie: either is right
+        assert tuple(big["idx"][:, i].tolist()) == best_idx, i
+        n_skip = sum(1 for t in best_idx if t < 0)
+        assert big["chi2"][i] + cfg["chi2_penalty"] * n_skip == pytest.approx(best_score, rel=1e-10, abs=1e-10)
+    assert n_multi >= 10
