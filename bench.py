@@ -432,6 +432,7 @@ def run_sweep(args):
     Bd.build()
     torch.cuda.set_device(0)
     stream = torch.cuda.current_stream()
+    cores = O.max_threads()                     # before any one-thread call (the OpenMP setting sticks)
     rows = []
     for name in ("tiny", "central", "central8", "pileup", "timeframe"):
         spec = W.CONFIGS[name]; data = W.generate(spec); cfg = W.matcher_config(spec)
@@ -461,13 +462,13 @@ def run_sweep(args):
         gpu_ms = e0.elapsed_time(e1) / steps
         B.trd_destroy(h)
         n_all = min(ORACLE_SAMPLE_TRACKS, n); n_1t = min(ORACLE_SAMPLE_TRACKS_1T, n)
-        ra = O.match(cfg, data, lo=0, hi=n_all)
+        ra = O.match(cfg, data, lo=0, hi=n_all, n_threads=cores)
         r1 = O.match(cfg, data, lo=0, hi=n_1t, n_threads=1)
         cpu_all_ms = 1e3 * (ra["seconds"]["index"] + ra["seconds"]["match"] * n / n_all)
         cpu_1t_ms = 1e3 * (r1["seconds"]["index"] + r1["seconds"]["match"] * n / n_1t)
         row = dict(sweep=name, n_tracks=n, n_tracklets=n_tl, n_hyp=spec.n_hyp, n_sigma_road=spec.n_sigma_road,
                    gpu_ms_per_step=gpu_ms, gpu_tracks_per_s=n / (gpu_ms * 1e-3), gpu_steps=steps,
-                   oracle_cores=O.max_threads(), oracle_all_cores_ms=cpu_all_ms, oracle_1_thread_ms=cpu_1t_ms,
+                   oracle_cores=cores, oracle_all_cores_ms=cpu_all_ms, oracle_1_thread_ms=cpu_1t_ms,
                    oracle_sample_tracks=[n_all, n_1t], unit="ms per step (load + match of the whole config)")
         rows.append(row)
         print(json.dumps(row), flush=True)

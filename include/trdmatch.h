@@ -160,7 +160,8 @@ typedef struct trd_index_info {
     int32_t n_passes;      /* 8-bit radix passes */
     int32_t n_interactions; /* 1 = no time-frame association */
     int32_t sort_kind;     /* 0 = radix sort, 1 = counting sort, 2 = counting sort met a long bin and the radix passes
-                              did the work (known only after a trd_copy_index of this load; 1 until then) */
+                              did the work (known only after a trd_copy_index of this load; 1 until then), 3 = the
+                              counting sort of small loads (up to 2^18 tracklets, index_sort = 0): one cooperative launch */
 } trd_index_info;
 
 typedef struct trd_handle trd_handle;

@@ -18,6 +18,8 @@
 // carries the z row (SURVEY.md 8(d).3 "design consequence"), and it uses (sector, layer)
 // rather than the chamber's stack, because the z window may straddle two stacks (reading R12).
 // All of it is HBM-streaming integer work; no tensor cores.
+#include <cooperative_groups.h>
+
 #include "trd_internal.cuh"
 
 namespace trd {
@@ -33,6 +35,17 @@ constexpr int kTile = kSortThreads * kItems;        // 4096 keys per tile
 
 // also packs (y, z, dy/dx, chamber) into one 16-byte record so that the gather after the sort reads
 // one sector per tracklet instead of three
+// a1: bin key of one tracklet; unusable tracklets (chamber or interaction out of range, y or z not finite) get n_bins
+// and sort behind every bin
+__device__ __forceinline__ uint32_t key_of(const IndexGeom& g, float yy, float zz, int ch, int ia) {
+    if (ch >= 0 && ch < g.n_chambers && isfinite(yy) && isfinite(zz) && ia >= 0 && ia < g.n_ia) {
+        const int sector = ch / g.per_sector, layer = ch % g.n_layers;
+        const uint32_t cell = (uint32_t)((ia * g.n_sectors + sector) * g.n_layers + layer);
+        return ((cell * (uint32_t)g.nz + (uint32_t)zrow_of(g, zz)) << g.nb_shift) + (uint32_t)ybin_of(g, yy);
+    }
+    return g.n_bins;
+}
+
 constexpr int kKeyItems = 8;                        // tracklets per thread
 __global__ void __launch_bounds__(256) tracklet_key(const float* __restrict__ y, const float* __restrict__ z,
                                                     const float* __restrict__ dydx, const int32_t* __restrict__ chamber,
@@ -52,13 +65,8 @@ __global__ void __launch_bounds__(256) tracklet_key(const float* __restrict__ y,
         const float yy = y[i], zz = z[i];
         const int ch = chamber[i];
         packed[i] = make_float4(yy, zz, dydx[i], __int_as_float(ch));
-        uint32_t k = g.n_bins;                          // unusable: behind every bin
         const int ia = (g.n_ia > 1) ? interaction[i] : 0;      // time-frame association: the interaction leads the key
-        if (ch >= 0 && ch < g.n_chambers && isfinite(yy) && isfinite(zz) && ia >= 0 && ia < g.n_ia) {
-            const int sector = ch / g.per_sector, layer = ch % g.n_layers;
-            const uint32_t cell = (uint32_t)((ia * g.n_sectors + sector) * g.n_layers + layer);
-            k = ((cell * (uint32_t)g.nz + (uint32_t)zrow_of(g, zz)) << g.nb_shift) + (uint32_t)ybin_of(g, yy);
-        }
+        const uint32_t k = key_of(g, yy, zz, ch, ia);
         key[i] = k;
         if (digit_tot) atomicAdd(&cnt[(k >> shift) & (kRadix - 1)], 1u);
     }
@@ -519,6 +527,246 @@ __global__ void __launch_bounds__(256) order_bins(const uint32_t* __restrict__ t
     }
 }
 
+// ---- small loads: the whole index in ONE cooperative launch ---------------------------------------------------------
+// An event of the paper's size (about 2000 tracks, here 7 000 - 240 000 tracklets) is launch bound: the
+// radix path is eleven launches of a few microseconds each.  This kernel runs the counting sort of the large loads as
+// phases of one grid, separated by grid barriers: zero the tables | key + count per bin | scan (three steps) | place
+// (atomic cursor per bin) | order every bin by the caller's position and record the z extents | long bins.  There is
+// no radix fallback behind it: a bin longer than kMaxBin is put in order by a whole block -- up to kSmallBitonic
+// tracklets by a bitonic sort in shared memory, longer ones (at most n / kSmallBitonic of them) by walking the caller's
+// arrays in order and writing the bin's members as they come.
+constexpr int64_t kSmallMax = 1 << 18;              // loads up to this many tracklets
+constexpr int kSmallThreads = 512;
+constexpr int kSmallScan = 8;                       // table entries per thread and chunk
+constexpr int kSmallChunk = kSmallThreads * kSmallScan;
+constexpr int kSmallBitonic = 4096;
+
+struct SmallIndex {
+    const float *y, *z, *dydx;
+    const int32_t *chamber, *interaction;
+    uint32_t* key;          // caller order (trd_copy_index)
+    float4* packed;         // caller order (trd_refit)
+    float4* store;
+    float* store_dx;
+    const float* chamber_dx;
+    uint32_t *tab, *cursor, *partial, *long_list, *long_count;
+    uint2* row_ext;
+    int64_t n;
+    uint32_t n_rows;
+    IndexGeom g;
+};
+
+__device__ __forceinline__ void row_extent(uint2* row_ext, uint32_t row, uint32_t zlo, uint32_t zhi) {
+    // called by whole warps; lanes without a row carry 0xffffffff and neutral extents
+    const uint32_t row0 = __reduce_min_sync(0xffffffffu, row);
+    if (__all_sync(0xffffffffu, row == row0 || row == 0xffffffffu)) {
+        zlo = __reduce_min_sync(0xffffffffu, zlo);
+        zhi = __reduce_max_sync(0xffffffffu, zhi);
+        if ((threadIdx.x & 31) == 0 && row0 != 0xffffffffu) {
+            atomicMin(&row_ext[row0].x, zlo);
+            atomicMax(&row_ext[row0].y, zhi);
+        }
+    } else if (row != 0xffffffffu) {
+        atomicMin(&row_ext[row].x, zlo);
+        atomicMax(&row_ext[row].y, zhi);
+    }
+}
+
+__global__ void __launch_bounds__(kSmallThreads) small_index(const SmallIndex a) {
+    namespace cg = cooperative_groups;
+    cg::grid_group grid = cg::this_grid();
+    __shared__ uint32_t warp_sums[32];
+    __shared__ uint32_t total;
+    __shared__ unsigned long long s_sort[kSmallBitonic];       // (position << 32 | slot) of a long bin
+    const IndexGeom& g = a.g;
+    const int64_t tid = (int64_t)blockIdx.x * kSmallThreads + threadIdx.x, n_thr = (int64_t)gridDim.x * kSmallThreads;
+    const int64_t m = (int64_t)g.n_bins + 3;                   // table entries; counts live at [key + 1]
+    const int n_chunks = (int)((m + kSmallChunk - 1) / kSmallChunk);
+    // ---- zero the tables
+    for (int64_t j = tid; j < m; j += n_thr) {
+        a.tab[j] = 0;
+        a.cursor[j] = 0;
+    }
+    if (a.row_ext)
+        for (int64_t j = tid; j < a.n_rows; j += n_thr) a.row_ext[j] = make_uint2(0xffffffffu, 0u);   // empty: min > max
+    if (tid == 0) *a.long_count = 0;
+    grid.sync();
+    // ---- a1: key, packed copy, count per bin
+    for (int64_t i = tid; i < a.n; i += n_thr) {
+        const float yy = a.y[i], zz = a.z[i];
+        const int ch = a.chamber[i];
+        const uint32_t k = key_of(g, yy, zz, ch, (g.n_ia > 1) ? a.interaction[i] : 0);
+        a.key[i] = k;
+        a.packed[i] = make_float4(yy, zz, a.dydx[i], __int_as_float(ch));
+        atomicAdd(a.tab + k + 1, 1u);
+    }
+    grid.sync();
+    // ---- a3: inclusive scan of the table -> tab[k] = first sorted position whose key is >= k
+    for (int c = blockIdx.x; c < n_chunks; c += gridDim.x) {
+        const int64_t base = (int64_t)c * kSmallChunk + (int64_t)threadIdx.x * kSmallScan;
+        uint32_t sum = 0;
+#pragma unroll
+        for (int u = 0; u < kSmallScan; ++u) sum += (base + u < m) ? a.tab[base + u] : 0u;
+        block_exclusive_scan(sum, warp_sums, &total);
+        if (threadIdx.x == 0) a.partial[c] = total;
+        __syncthreads();
+    }
+    grid.sync();
+    if (blockIdx.x == 0) {
+        uint32_t carry = 0;
+        for (int t0 = 0; t0 < n_chunks; t0 += kSmallThreads) {
+            const int t = t0 + threadIdx.x;
+            const uint32_t v = (t < n_chunks) ? a.partial[t] : 0u;
+            const uint32_t ex = block_exclusive_scan(v, warp_sums, &total);
+            if (t < n_chunks) a.partial[t] = carry + ex;
+            carry += total;
+            __syncthreads();
+        }
+    }
+    grid.sync();
+    for (int c = blockIdx.x; c < n_chunks; c += gridDim.x) {
+        const int64_t base = (int64_t)c * kSmallChunk + (int64_t)threadIdx.x * kSmallScan;
+        uint32_t v[kSmallScan];
+#pragma unroll
+        for (int u = 0; u < kSmallScan; ++u) v[u] = (base + u < m) ? a.tab[base + u] : 0u;
+#pragma unroll
+        for (int u = 1; u < kSmallScan; ++u) v[u] += v[u - 1];
+        const uint32_t off = a.partial[c] + block_exclusive_scan(v[kSmallScan - 1], warp_sums, &total);
+#pragma unroll
+        for (int u = 0; u < kSmallScan; ++u)
+            if (base + u < m) a.tab[base + u] = v[u] + off;
+        __syncthreads();
+    }
+    grid.sync();
+    // ---- a2: every tracklet to the next free place of its bin (order inside the bin restored below)
+    for (int64_t i = tid; i < a.n; i += n_thr) {
+        const uint32_t k = a.key[i];
+        const uint32_t pos = a.tab[k] + atomicAdd(a.cursor + k, 1u);
+        const float4 tl = a.packed[i];
+        a.store[pos] = make_float4(tl.x, tl.y, tl.z, __uint_as_float((uint32_t)i));
+        if (a.store_dx) {
+            const int ch = __float_as_int(tl.w);
+            a.store_dx[pos] = (ch >= 0 && ch < g.n_chambers) ? __ldg(a.chamber_dx + ch) : 0.0f;
+        }
+    }
+    grid.sync();
+    // ---- the caller's order inside every bin, z extent of every row; long bins go on a list
+    const int64_t n_bins_up = ((int64_t)g.n_bins + 31) / 32 * 32;
+    for (int64_t b = tid; b < n_bins_up; b += n_thr) {
+        uint32_t row = 0xffffffffu, zlo = 0xffffffffu, zhi = 0u;
+        if (b < g.n_bins) {
+            const uint32_t s0 = a.tab[b], e = a.tab[b + 1];
+            if (e - s0 > (uint32_t)kMaxBin) {
+                a.long_list[atomicAdd(a.long_count, 1u)] = (uint32_t)b;
+            } else if (e > s0) {
+                float4 prev = a.store[s0];
+                row = (uint32_t)(b >> g.nb_shift);
+                zlo = zhi = ext_encode(prev.y);
+                for (uint32_t i = s0 + 1; i < e; ++i) {
+                    float4 v = a.store[i];
+                    const uint32_t z = ext_encode(v.y);
+                    zlo = min(zlo, z);
+                    zhi = max(zhi, z);
+                    if (__float_as_uint(prev.w) > __float_as_uint(v.w)) {       // out of order: sink v
+                        const float dxv = a.store_dx ? a.store_dx[i] : 0.0f;
+                        uint32_t j = i;
+                        while (j > s0) {
+                            const float4 u = a.store[j - 1];
+                            if (__float_as_uint(u.w) < __float_as_uint(v.w)) break;
+                            a.store[j] = u;
+                            if (a.store_dx) a.store_dx[j] = a.store_dx[j - 1];
+                            --j;
+                        }
+                        a.store[j] = v;
+                        if (a.store_dx) a.store_dx[j] = dxv;
+                        v = a.store[i];
+                    }
+                    prev = v;
+                }
+            }
+        }
+        if (a.row_ext) row_extent(a.row_ext, row, zlo, zhi);
+    }
+    grid.sync();
+    // ---- long bins: one block each
+    const uint32_t n_long = *a.long_count;
+    for (uint32_t q = blockIdx.x; q < n_long; q += gridDim.x) {
+        const uint32_t b = a.long_list[q];
+        const uint32_t s0 = a.tab[b], c = a.tab[b + 1] - s0;
+        if (a.row_ext) {                                             // z extent of the bin's row
+            for (uint32_t i0 = 0; i0 < c; i0 += kSmallThreads) {
+                const uint32_t i = i0 + threadIdx.x;
+                uint32_t zlo = 0xffffffffu, zhi = 0u, row = 0xffffffffu;
+                if (i < c) {
+                    zlo = zhi = ext_encode(a.store[s0 + i].y);
+                    row = b >> g.nb_shift;
+                }
+                row_extent(a.row_ext, row, zlo, zhi);
+            }
+        }
+        if (c <= (uint32_t)kSmallBitonic) {
+            // (position, slot) pairs sorted in shared memory; then every place takes the record of its rank
+            for (uint32_t i = threadIdx.x; i < (uint32_t)kSmallBitonic; i += kSmallThreads)
+                s_sort[i] = (i < c) ? (((unsigned long long)__float_as_uint(a.store[s0 + i].w) << 32) | i) : ~0ull;
+            __syncthreads();
+            for (uint32_t k2 = 2; k2 <= (uint32_t)kSmallBitonic; k2 <<= 1)
+                for (uint32_t j = k2 >> 1; j > 0; j >>= 1) {
+                    for (uint32_t i = threadIdx.x; i < (uint32_t)kSmallBitonic; i += kSmallThreads) {
+                        const uint32_t l = i ^ j;
+                        if (l > i) {
+                            const unsigned long long x = s_sort[i], w = s_sort[l];
+                            if (((i & k2) == 0) ? (x > w) : (x < w)) {
+                                s_sort[i] = w;
+                                s_sort[l] = x;
+                            }
+                        }
+                    }
+                    __syncthreads();
+                }
+            // gather: rank r takes the record that sits in slot (s_sort[r] & 0xffffffff); read all, sync, write all
+            float4 rec[kSmallBitonic / kSmallThreads];
+            float dxs[kSmallBitonic / kSmallThreads];
+#pragma unroll
+            for (int u = 0; u < kSmallBitonic / kSmallThreads; ++u) {
+                const uint32_t r = u * kSmallThreads + threadIdx.x;
+                if (r < c) {
+                    const uint32_t slot = (uint32_t)(s_sort[r] & 0xffffffffull);
+                    rec[u] = a.store[s0 + slot];
+                    dxs[u] = a.store_dx ? a.store_dx[s0 + slot] : 0.0f;
+                }
+            }
+            __syncthreads();
+#pragma unroll
+            for (int u = 0; u < kSmallBitonic / kSmallThreads; ++u) {
+                const uint32_t r = u * kSmallThreads + threadIdx.x;
+                if (r < c) {
+                    a.store[s0 + r] = rec[u];
+                    if (a.store_dx) a.store_dx[s0 + r] = dxs[u];
+                }
+            }
+            __syncthreads();
+        } else {
+            // walk the caller's arrays in order: the members of the bin come out in the caller's order
+            uint32_t done = 0;
+            for (int64_t i0 = 0; i0 < a.n; i0 += kSmallThreads) {
+                const int64_t i = i0 + threadIdx.x;
+                const bool mine = i < a.n && a.key[i] == b;
+                const uint32_t ex = block_exclusive_scan(mine ? 1u : 0u, warp_sums, &total);
+                if (mine) {
+                    const float4 tl = a.packed[i];
+                    a.store[s0 + done + ex] = make_float4(tl.x, tl.y, tl.z, __uint_as_float((uint32_t)i));
+                    if (a.store_dx) {
+                        const int ch = __float_as_int(tl.w);
+                        a.store_dx[s0 + done + ex] = (ch >= 0 && ch < g.n_chambers) ? __ldg(a.chamber_dx + ch) : 0.0f;
+                    }
+                }
+                done += total;
+                __syncthreads();
+            }
+        }
+    }
+}
+
 // trd_copy_index after a counting sort: the sorted positions and keys the radix path leaves behind
 __global__ void __launch_bounds__(256) export_sorted(const float4* __restrict__ store, const uint32_t* __restrict__ key,
                                                      uint32_t* __restrict__ sorted_pos, uint32_t* __restrict__ sorted_key, int64_t n) {
@@ -587,13 +835,15 @@ cudaError_t radix_sort_pairs(uint32_t* key0, uint32_t* key1, uint32_t* val0, uin
 
 // trd_copy_index: sorted positions and keys into val[sorted_side] / key[sorted_side] when the counting sort built the store
 cudaError_t export_sorted_index(trd_handle* h, cudaStream_t stream) {
-    if (h->sort_kind != 1 || h->n_tracklets == 0) return cudaSuccess;
+    if ((h->sort_kind != 1 && h->sort_kind != 3) || h->n_tracklets == 0) return cudaSuccess;
     int flag = 0;
+    if (h->sort_kind == 1) {
     TRD_TRY(cudaMemcpyAsync(&flag, h->sort_flag.p, sizeof(int), cudaMemcpyDeviceToHost, stream));
     TRD_TRY(cudaStreamSynchronize(stream));
     if (flag != 0) {                                   // a bin was too long: the radix kernels did the work
         h->sort_kind = 2;
         return cudaSuccess;
+    }
     }
     const int64_t n = h->n_tracklets;
     h->sorted_side = 1;
@@ -654,15 +904,64 @@ cudaError_t build_index(trd_handle* h, const float* d_y, const float* d_z, const
     if (h->use_row_ext) {
         const size_t n_rows = (size_t)n_cells * g.nz;
         TRD_TRY(reserve(h->row_ext, n_rows * sizeof(uint2), stream));
-        // empty rows: min = 0xffffffff > max = 0
-        TRD_TRY(cudaMemset2DAsync(h->row_ext.p, sizeof(uint2), 0xff, sizeof(uint32_t), n_rows, stream));
-        TRD_TRY(cudaMemset2DAsync((char*)h->row_ext.p + sizeof(uint32_t), sizeof(uint2), 0x00, sizeof(uint32_t), n_rows, stream));
     }
     if (n == 0) {
         TRD_TRY(cudaMemsetAsync(h->bin_first.p, 0, n_tab * sizeof(int32_t), stream));
         h->sort_kind = 0;
         h->index_loaded = true;
         return cudaSuccess;
+    }
+    if (c.index_sort == 0 && n <= kSmallMax) {
+        // small load: the whole index in one cooperative launch (small_index)
+        const bool has_dx_s = h->mp.dx_max > 0.0f;
+        TRD_TRY(reserve(h->store, (size_t)n * sizeof(float4), stream));
+        TRD_TRY(reserve(h->packed, (size_t)n * sizeof(float4), stream));
+        if (has_dx_s) TRD_TRY(reserve(h->store_dx, (size_t)n * sizeof(float), stream));
+        TRD_TRY(reserve(h->key[0], (size_t)n * sizeof(uint32_t), stream));
+        TRD_TRY(reserve(h->val[0], (size_t)n * sizeof(uint32_t), stream));              // list of long bins
+        TRD_TRY(reserve(h->key[1], (size_t)n * sizeof(uint32_t), stream));              // trd_copy_index exports into these two
+        TRD_TRY(reserve(h->val[1], (size_t)n * sizeof(uint32_t), stream));
+        TRD_TRY(reserve(h->tile_hist, n_tab * sizeof(uint32_t), stream));               // placement cursors
+        const int n_chunks = (int)((n_tab + kSmallChunk - 1) / kSmallChunk);
+        TRD_TRY(reserve(h->scan_partial, (size_t)n_chunks * sizeof(uint32_t), stream));
+        TRD_TRY(reserve(h->sort_flag, sizeof(int), stream));
+        if (h->small_grid == 0) {
+            int per_sm = 0;
+            TRD_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, small_index, kSmallThreads, 0));
+            h->small_grid = per_sm * h->sm_count;
+            if (h->small_grid < 1) return cudaErrorLaunchOutOfResources;
+        }
+        SmallIndex a;
+        a.y = d_y; a.z = d_z; a.dydx = d_dydx; a.chamber = d_chamber; a.interaction = d_interaction;
+        a.key = (uint32_t*)h->key[0].p;
+        a.packed = (float4*)h->packed.p;
+        a.store = (float4*)h->store.p;
+        a.store_dx = has_dx_s ? (float*)h->store_dx.p : nullptr;
+        a.chamber_dx = has_dx_s ? (const float*)h->chamber_dx.p : nullptr;
+        a.tab = (uint32_t*)h->bin_first.p;
+        a.cursor = (uint32_t*)h->tile_hist.p;
+        a.partial = (uint32_t*)h->scan_partial.p;
+        a.long_list = (uint32_t*)h->val[0].p;
+        a.long_count = (uint32_t*)h->sort_flag.p;
+        a.row_ext = h->use_row_ext ? (uint2*)h->row_ext.p : nullptr;
+        a.n = n;
+        a.n_rows = (uint32_t)(n_cells * g.nz);
+        a.g = g;
+        const int64_t work = n_tab > (size_t)n ? (int64_t)n_tab : n;
+        int grid = (int)((work + kSmallThreads - 1) / kSmallThreads);
+        if (grid > h->small_grid) grid = h->small_grid;
+        void* args[] = {&a};
+        TRD_TRY(cudaLaunchCooperativeKernel((const void*)small_index, dim3((unsigned)grid), dim3(kSmallThreads), args, 0, stream));
+        h->launches++;
+        h->sort_kind = 3;
+        h->sorted_side = 1;
+        h->index_loaded = true;
+        return cudaSuccess;
+    }
+    if (h->use_row_ext) {                                 // empty rows: min = 0xffffffff > max = 0
+        const size_t n_rows = (size_t)n_cells * g.nz;
+        TRD_TRY(cudaMemset2DAsync(h->row_ext.p, sizeof(uint2), 0xff, sizeof(uint32_t), n_rows, stream));
+        TRD_TRY(cudaMemset2DAsync((char*)h->row_ext.p + sizeof(uint32_t), sizeof(uint2), 0x00, sizeof(uint32_t), n_rows, stream));
     }
     const int n_tiles = (int)((n + kTile - 1) / kTile);
     TRD_TRY(reserve(h->store, (size_t)n * sizeof(float4), stream));

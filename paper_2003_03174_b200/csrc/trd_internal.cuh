@@ -113,7 +113,9 @@ struct trd_handle {
     trd::Buffer chamber_dx; // float per chamber: radial offset from the nominal layer plane (trd_set_chamber_dx)
     trd::Buffer store_dx;   // float per sorted tracklet: the offset of its chamber (only when offsets are set)
     int sorted_side = 0;    // which of key[]/val[] holds the sorted result
-    int sort_kind = 0;      // last load: 0 = radix sort, 1 = counting sort, 2 = counting sort gave up (long bin), radix did it
+    int sort_kind = 0;      // last load: 0 = radix sort, 1 = counting sort, 2 = counting sort gave up (long bin), radix did it,
+                            // 3 = counting sort in one cooperative launch (small loads)
+    int small_grid = 0;     // blocks of the cooperative launch (occupancy x SMs), found on first use
     trd::Buffer sort_flag;  // int: set by the counting sort when a bin is too long for it
     trd::Buffer scan_partial;  // chunk sums of the count table
     trd::Buffer part_rec;   // counting sort: float4 per tracklet, partitioned by the leading key digit

@@ -41,7 +41,7 @@ def check_index(cfg, ix, y, z, ch):
     key_of_input = np.empty(n, np.int64); key_of_input[pos] = key
     ref = np.argsort(key_of_input, kind="stable")
     assert np.array_equal(pos[:n_usable], ref[:n_usable])
-    if ix["sort_kind"] == 1:
+    if ix["sort_kind"] in (1, 3):
         assert np.array_equal(np.sort(pos[n_usable:]), ref[n_usable:])        # the unusable ones: any order
     else:
         assert np.array_equal(pos, ref)
@@ -96,14 +96,16 @@ def test_ragged_sizes_and_unusable_tracklets(B, base_cfg, n, ybin_width, index_s
     h, ix = load(B, cfg, y, z, d, ch)
     try:
         check_index(cfg, ix, y, z, ch)
-        assert ix["sort_kind"] == (1 if index_sort > 0 or (index_sort == 0 and n >= 1 << 18) else 0)
+        # index_sort = 0: up to 2^18 tracklets the counting sort runs as one cooperative launch (3), above it as the
+        # multi-kernel counting sort (1)
+        assert ix["sort_kind"] == (1 if index_sort > 0 or (index_sort == 0 and n > 1 << 18) else (3 if index_sort == 0 else 0))
         if ybin_width > 0:
             assert ix["ybin_width"] <= ybin_width
     finally:
         B.trd_destroy(h)
 
 
-@pytest.mark.parametrize("index_sort", [-1, 1])
+@pytest.mark.parametrize("index_sort", [-1, 0, 1])
 def test_skewed_keys_one_bin_and_reload(B, base_cfg, index_sort):
     """All tracklets in one bin (worst case for the scatter ranks; the counting sort hands a bin this long to the
     radix passes on the device), then a smaller reload on the same handle."""
@@ -116,7 +118,7 @@ def test_skewed_keys_one_bin_and_reload(B, base_cfg, index_sort):
     try:
         check_index(base_cfg, ix, y, z, ch)
         assert np.array_equal(ix["sorted_pos"], np.arange(n))
-        assert ix["sort_kind"] == (2 if index_sort > 0 else 0)
+        assert ix["sort_kind"] == {1: 2, 0: 3, -1: 0}[index_sort]   # 3: the one-launch sort orders the long bin itself
         t = [torch.from_numpy(a[:100].copy()).cuda() for a in (y, z, d, ch)]
         B.trd_load_tracklets(h, *t)
         ix2 = B.trd_copy_index(h)
@@ -146,5 +148,28 @@ def test_counting_sort_keeps_the_callers_order_inside_a_bin(B, base_cfg, n_dup):
         check_index(cfg, ix, y, z, ch)
         longest = np.diff(ix["bin_first"].astype(np.int64)).max()         # two groups may share a bin
         assert longest >= n_dup and ix["sort_kind"] == (1 if longest <= 32 else 2)
+    finally:
+        B.trd_destroy(h)
+
+
+@pytest.mark.parametrize("n_groups,n_dup", [(5000, 33), (300, 700), (60, 4096), (40, 5000), (3, 80_000)])
+def test_one_launch_sort_orders_long_bins_itself(B, base_cfg, n_groups, n_dup):
+    """Small loads (index_sort = 0, up to 2^18 tracklets) are indexed by ONE cooperative launch with no radix passes
+    behind it: bins longer than 32 are put into the caller's order by a whole block -- a bitonic sort in shared memory
+    up to 4096 tracklets, a walk over the caller's arrays beyond."""
+    rng = np.random.default_rng(n_dup)
+    ch_g = rng.integers(0, 540, n_groups).astype(np.int32)
+    y_g = rng.uniform(-50, 50, n_groups).astype(np.float32); z_g = (8.0 * rng.integers(-40, 40, n_groups) + 4.0).astype(np.float32)
+    order = rng.permutation(n_groups * n_dup)
+    g = (np.arange(n_groups * n_dup) // n_dup)[order]
+    y, z, ch = y_g[g], z_g[g], ch_g[g]
+    d = rng.uniform(-0.5, 0.5, g.size).astype(np.float32)
+    assert g.size <= 1 << 18
+    cfg = dict(base_cfg, index_sort=0)
+    h, ix = load(B, cfg, y, z, d, ch)
+    try:
+        check_index(cfg, ix, y, z, ch)
+        assert ix["sort_kind"] == 3
+        assert np.diff(ix["bin_first"].astype(np.int64)).max() >= n_dup
     finally:
         B.trd_destroy(h)
