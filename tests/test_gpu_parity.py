@@ -54,6 +54,7 @@ def run_gpu(B, cfg, data, batch=None, in_place=False):
 
 
 FLIPS = []       # (what, tracks, fragile tracks, flipped chains) of every comparison of this session, printed at the end
+STATS = dict(max_replays=0, chi2_max_rel_err=0.0, par_max_scaled_err=0.0)
 
 
 def check_parity(got, want, cfg, data, lo=0, what="", max_flip_frac=0.25, record=True, **tol):
@@ -66,6 +67,8 @@ def check_parity(got, want, cfg, data, lo=0, what="", max_flip_frac=0.25, record
     rep = P.compare(got, want, **tol)
     assert rep["ok"], {k: v for k, v in rep.items()}
     assert rep["n_evals_bad"] == 0
+    STATS["chi2_max_rel_err"] = max(STATS["chi2_max_rel_err"], rep["chi2_max_rel_err"])
+    STATS["par_max_scaled_err"] = max(STATS["par_max_scaled_err"], max(rep["par_max_scaled_err"]))
     flips = rep["flip_tracks"]
     if record:
         FLIPS.append((what, rep["n_tracks"], rep["n_fragile"], int(flips.shape[0])))
@@ -75,6 +78,7 @@ def check_parity(got, want, cfg, data, lo=0, what="", max_flip_frac=0.25, record
         tol2 = {k: v for k, v in tol.items() if k != "eps_margin"}
         rep2 = P.compare_alternatives({k: v[..., :n] for k, v in got.items()}, alt, flips, **tol2)
         assert rep2["ok"], {k: v for k, v in rep2.items()}
+        STATS["max_replays"] = max(STATS["max_replays"], rep2["max_replays"])
         assert flips.shape[0] <= max(3, max_flip_frac * rep["n_fragile"]), (flips.shape[0], rep["n_fragile"])
     return rep
 
@@ -84,7 +88,9 @@ def _report_flips():
     yield
     tot = [sum(f[k] for f in FLIPS) for k in (1, 2, 3)]
     print(f"\n[parity] {len(FLIPS)} comparisons, {tot[0]} tracks, {tot[1]} fragile (margin < 1e-4), {tot[2]} flipped chains, "
-          f"every one validated as an alternative result of the oracle")
+          f"every one validated as an alternative result of the oracle (at most {STATS['max_replays']} replays); "
+          f"chi2 max rel. error {STATS['chi2_max_rel_err']:.2e}, parameter error at most {STATS['par_max_scaled_err']:.2e} of "
+          f"max(|p|, 0.1) on tracks with equal chains")
     for what, n, nf, nfl in FLIPS:
         if what:
             print(f"[parity] {what}: {n} tracks, {nf} fragile, {nfl} flips")
