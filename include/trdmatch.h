@@ -105,8 +105,8 @@ typedef struct trd_config {
     int32_t index_sort;              /* how trd_load_tracklets orders the tracklets by bin: 0 = counting sort (count per bin,
                                         scan, placement, caller's order restored inside every bin) for loads of 2^18
                                         tracklets or more, 8-bit radix passes below; 1 = counting sort always; -1 = radix
-                                        always.  A bin of more than 32 tracklets sends the whole load through the radix
-                                        passes (decided on the device).  The index is the same either way, except for the
+                                        always.  A bin of more than 32 tracklets sends the whole load through the
+                                        one-launch sort of small loads, which orders long bins itself (decided on the device).  The index is the same either way, except for the
                                         order of the unusable tracklets behind the last bin, which nothing reads. */
     int32_t reserved_;
 } trd_config;
@@ -159,8 +159,8 @@ typedef struct trd_index_info {
     int32_t key_bits;      /* radix-sorted key width */
     int32_t n_passes;      /* 8-bit radix passes */
     int32_t n_interactions; /* 1 = no time-frame association */
-    int32_t sort_kind;     /* 0 = radix sort, 1 = counting sort, 2 = counting sort met a long bin and the radix passes
-                              did the work (known only after a trd_copy_index of this load; 1 until then), 3 = the
+    int32_t sort_kind;     /* 0 = radix sort, 1 = counting sort, 2 = counting sort met a long bin and the one-launch
+                              sort did the work (known only after a trd_copy_index of this load; 1 until then), 3 = the
                               counting sort of small loads (up to 2^18 tracklets, index_sort = 0): one cooperative launch */
 } trd_index_info;
 

@@ -550,6 +550,7 @@ struct SmallIndex {
     float* store_dx;
     const float* chamber_dx;
     uint32_t *tab, *cursor, *partial, *long_list, *long_count;
+    const int* gate;        // when given, the kernel runs only if *gate != 0 (fallback of the multi-kernel counting sort)
     uint2* row_ext;
     int64_t n;
     uint32_t n_rows;
@@ -578,6 +579,7 @@ __global__ void __launch_bounds__(kSmallThreads) small_index(const SmallIndex a)
     __shared__ uint32_t warp_sums[32];
     __shared__ uint32_t total;
     __shared__ unsigned long long s_sort[kSmallBitonic];       // (position << 32 | slot) of a long bin
+    if (a.gate && *a.gate == 0) return;                        // every block: nobody reaches a grid barrier
     const IndexGeom& g = a.g;
     const int64_t tid = (int64_t)blockIdx.x * kSmallThreads + threadIdx.x, n_thr = (int64_t)gridDim.x * kSmallThreads;
     const int64_t m = (int64_t)g.n_bins + 3;                   // table entries; counts live at [key + 1]
@@ -840,10 +842,7 @@ cudaError_t export_sorted_index(trd_handle* h, cudaStream_t stream) {
     if (h->sort_kind == 1) {
     TRD_TRY(cudaMemcpyAsync(&flag, h->sort_flag.p, sizeof(int), cudaMemcpyDeviceToHost, stream));
     TRD_TRY(cudaStreamSynchronize(stream));
-    if (flag != 0) {                                   // a bin was too long: the radix kernels did the work
-        h->sort_kind = 2;
-        return cudaSuccess;
-    }
+    if (flag != 0) h->sort_kind = 2;                   // a bin was too long: the one-launch sort did the work
     }
     const int64_t n = h->n_tracklets;
     h->sorted_side = 1;
@@ -851,6 +850,56 @@ cudaError_t export_sorted_index(trd_handle* h, cudaStream_t stream) {
                                                                   (uint32_t*)h->val[1].p, (uint32_t*)h->key[1].p, n);
     TRD_TRY(cudaGetLastError());
     return cudaStreamSynchronize(stream);
+}
+
+// the whole index in one cooperative launch; with `gate` the launch is the fallback of the multi-kernel counting sort
+// and does nothing unless the device flag is set
+static cudaError_t launch_small_index(trd_handle* h, const float* d_y, const float* d_z, const float* d_dydx, const int32_t* d_chamber,
+                                      const int32_t* d_interaction, int64_t n, size_t n_tab, int64_t n_cells, const int* gate,
+                                      cudaStream_t stream) {
+    const IndexGeom& g = h->mp.g;
+    const bool has_dx = h->mp.dx_max > 0.0f;
+    TRD_TRY(reserve(h->store, (size_t)n * sizeof(float4), stream));
+    TRD_TRY(reserve(h->packed, (size_t)n * sizeof(float4), stream));
+    if (has_dx) TRD_TRY(reserve(h->store_dx, (size_t)n * sizeof(float), stream));
+    for (int sd = 0; sd < 2; ++sd) {                                  // [0]: keys in caller order / list of long bins;
+        TRD_TRY(reserve(h->key[sd], (size_t)n * sizeof(uint32_t), stream));   // [1]: trd_copy_index exports into these
+        TRD_TRY(reserve(h->val[sd], (size_t)n * sizeof(uint32_t), stream));
+    }
+    TRD_TRY(reserve(h->tile_hist, n_tab * sizeof(uint32_t), stream));               // placement cursors
+    const int n_chunks = (int)((n_tab + kSmallChunk - 1) / kSmallChunk);
+    TRD_TRY(reserve(h->scan_partial, (size_t)n_chunks * sizeof(uint32_t), stream));
+    TRD_TRY(reserve(h->sort_flag, 2 * sizeof(int), stream));
+    if (h->small_grid == 0) {
+        int per_sm = 0;
+        TRD_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, small_index, kSmallThreads, 0));
+        h->small_grid = per_sm * h->sm_count;
+        if (h->small_grid < 1) return cudaErrorLaunchOutOfResources;
+    }
+    SmallIndex a;
+    a.y = d_y; a.z = d_z; a.dydx = d_dydx; a.chamber = d_chamber; a.interaction = d_interaction;
+    a.key = (uint32_t*)h->key[0].p;
+    a.packed = (float4*)h->packed.p;
+    a.store = (float4*)h->store.p;
+    a.store_dx = has_dx ? (float*)h->store_dx.p : nullptr;
+    a.chamber_dx = has_dx ? (const float*)h->chamber_dx.p : nullptr;
+    a.tab = (uint32_t*)h->bin_first.p;
+    a.cursor = (uint32_t*)h->tile_hist.p;
+    a.partial = (uint32_t*)h->scan_partial.p;
+    a.long_list = (uint32_t*)h->val[0].p;
+    a.long_count = (uint32_t*)h->sort_flag.p + 1;
+    a.gate = gate;
+    a.row_ext = h->use_row_ext ? (uint2*)h->row_ext.p : nullptr;
+    a.n = n;
+    a.n_rows = (uint32_t)(n_cells * g.nz);
+    a.g = g;
+    const int64_t work = n_tab > (size_t)n ? (int64_t)n_tab : n;
+    int grid = (int)((work + kSmallThreads - 1) / kSmallThreads);
+    if (grid > h->small_grid) grid = h->small_grid;
+    void* args[] = {&a};
+    TRD_TRY(cudaLaunchCooperativeKernel((const void*)small_index, dim3((unsigned)grid), dim3(kSmallThreads), args, 0, stream));
+    h->launches++;
+    return cudaSuccess;
 }
 
 cudaError_t build_index(trd_handle* h, const float* d_y, const float* d_z, const float* d_dydx,
@@ -913,46 +962,7 @@ cudaError_t build_index(trd_handle* h, const float* d_y, const float* d_z, const
     }
     if (c.index_sort == 0 && n <= kSmallMax) {
         // small load: the whole index in one cooperative launch (small_index)
-        const bool has_dx_s = h->mp.dx_max > 0.0f;
-        TRD_TRY(reserve(h->store, (size_t)n * sizeof(float4), stream));
-        TRD_TRY(reserve(h->packed, (size_t)n * sizeof(float4), stream));
-        if (has_dx_s) TRD_TRY(reserve(h->store_dx, (size_t)n * sizeof(float), stream));
-        TRD_TRY(reserve(h->key[0], (size_t)n * sizeof(uint32_t), stream));
-        TRD_TRY(reserve(h->val[0], (size_t)n * sizeof(uint32_t), stream));              // list of long bins
-        TRD_TRY(reserve(h->key[1], (size_t)n * sizeof(uint32_t), stream));              // trd_copy_index exports into these two
-        TRD_TRY(reserve(h->val[1], (size_t)n * sizeof(uint32_t), stream));
-        TRD_TRY(reserve(h->tile_hist, n_tab * sizeof(uint32_t), stream));               // placement cursors
-        const int n_chunks = (int)((n_tab + kSmallChunk - 1) / kSmallChunk);
-        TRD_TRY(reserve(h->scan_partial, (size_t)n_chunks * sizeof(uint32_t), stream));
-        TRD_TRY(reserve(h->sort_flag, sizeof(int), stream));
-        if (h->small_grid == 0) {
-            int per_sm = 0;
-            TRD_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, small_index, kSmallThreads, 0));
-            h->small_grid = per_sm * h->sm_count;
-            if (h->small_grid < 1) return cudaErrorLaunchOutOfResources;
-        }
-        SmallIndex a;
-        a.y = d_y; a.z = d_z; a.dydx = d_dydx; a.chamber = d_chamber; a.interaction = d_interaction;
-        a.key = (uint32_t*)h->key[0].p;
-        a.packed = (float4*)h->packed.p;
-        a.store = (float4*)h->store.p;
-        a.store_dx = has_dx_s ? (float*)h->store_dx.p : nullptr;
-        a.chamber_dx = has_dx_s ? (const float*)h->chamber_dx.p : nullptr;
-        a.tab = (uint32_t*)h->bin_first.p;
-        a.cursor = (uint32_t*)h->tile_hist.p;
-        a.partial = (uint32_t*)h->scan_partial.p;
-        a.long_list = (uint32_t*)h->val[0].p;
-        a.long_count = (uint32_t*)h->sort_flag.p;
-        a.row_ext = h->use_row_ext ? (uint2*)h->row_ext.p : nullptr;
-        a.n = n;
-        a.n_rows = (uint32_t)(n_cells * g.nz);
-        a.g = g;
-        const int64_t work = n_tab > (size_t)n ? (int64_t)n_tab : n;
-        int grid = (int)((work + kSmallThreads - 1) / kSmallThreads);
-        if (grid > h->small_grid) grid = h->small_grid;
-        void* args[] = {&a};
-        TRD_TRY(cudaLaunchCooperativeKernel((const void*)small_index, dim3((unsigned)grid), dim3(kSmallThreads), args, 0, stream));
-        h->launches++;
+        TRD_TRY(launch_small_index(h, d_y, d_z, d_dydx, d_chamber, d_interaction, n, n_tab, n_cells, nullptr, stream));
         h->sort_kind = 3;
         h->sorted_side = 1;
         h->index_loaded = true;
@@ -985,7 +995,7 @@ cudaError_t build_index(trd_handle* h, const float* d_y, const float* d_z, const
     h->launches++;
     if (counting) {
         const int n_chunks = (int)((n_tab + kScanChunk - 1) / kScanChunk);
-        TRD_TRY(reserve(h->sort_flag, sizeof(int), stream));
+        TRD_TRY(reserve(h->sort_flag, 2 * sizeof(int), stream));
         TRD_TRY(reserve(h->scan_partial, (size_t)n_chunks * sizeof(uint32_t), stream));
         TRD_TRY(reserve(h->part_rec, (size_t)n * sizeof(float4), stream));
         if (has_dx) TRD_TRY(reserve(h->part_dx, (size_t)n * sizeof(float), stream));
@@ -1016,14 +1026,22 @@ cudaError_t build_index(trd_handle* h, const float* d_y, const float* d_z, const
         TRD_TRY(cudaGetLastError());
         gate = flag;                                     // the radix kernels below run only if a bin was too long
     }
+    if (gate) {
+        // a bin longer than kMaxBin made the counting kernels return: the one-launch sort, which orders long bins itself,
+        // does the load again (gated on the same device flag: one idle launch otherwise)
+        TRD_TRY(launch_small_index(h, d_y, d_z, d_dydx, d_chamber, d_interaction, n, n_tab, n_cells, gate, stream));
+        h->sorted_side = 1;
+        h->index_loaded = true;
+        return cudaSuccess;
+    }
     int side = 0;
     TRD_TRY(radix_sort_pairs((uint32_t*)h->key[0].p, (uint32_t*)h->key[1].p, (uint32_t*)h->val[0].p, (uint32_t*)h->val[1].p,
-                             (uint32_t*)h->tile_hist.p, (uint32_t*)h->digit_tot.p, n, h->n_passes, stream, &side, &h->launches, gate));
+                             (uint32_t*)h->tile_hist.p, (uint32_t*)h->digit_tot.p, n, h->n_passes, stream, &side, &h->launches, nullptr));
     h->sorted_side = side;
     gather_store<<<(unsigned)((n + 256 * kGather - 1) / (256 * kGather)), 256, 0, stream>>>((const uint32_t*)h->val[side].p, (const uint32_t*)h->key[side].p,
                                            (const float4*)h->packed.p, (float4*)h->store.p, h->use_row_ext ? (uint2*)h->row_ext.p : nullptr,
                                            (int32_t*)h->bin_first.p, has_dx ? (const float*)h->chamber_dx.p : nullptr,
-                                           has_dx ? (float*)h->store_dx.p : nullptr, g.n_chambers, n, g.n_bins, g.nb_shift, gate);
+                                           has_dx ? (float*)h->store_dx.p : nullptr, g.n_chambers, n, g.n_bins, g.nb_shift, nullptr);
     h->launches += 1;
     TRD_TRY(cudaGetLastError());
     h->index_loaded = true;
