@@ -103,11 +103,13 @@ typedef struct trd_config {
      * outer corner. */
     double bz_r2, bz_z2;             /* [1/cm^2] */
     int32_t index_sort;              /* how trd_load_tracklets orders the tracklets by bin: 0 = counting sort (count per bin,
-                                        scan, placement, caller's order restored inside every bin) for loads of 2^18
-                                        tracklets or more, 8-bit radix passes below; 1 = counting sort always; -1 = radix
-                                        always.  A bin of more than 32 tracklets sends the whole load through the
-                                        one-launch sort of small loads, which orders long bins itself (decided on the device).  The index is the same either way, except for the
-                                        order of the unusable tracklets behind the last bin, which nothing reads. */
+                                        scan, placement, caller's order restored inside every bin): several kernels for
+                                        loads above 2^18 tracklets, one cooperative launch up to that size; 1 = the
+                                        several-kernel counting sort always; -1 = 8-bit radix passes always.  A bin of more
+                                        than 32 tracklets sends a large load through the one-launch sort, which orders
+                                        long bins itself (decided on the device).  The index is the same either way,
+                                        except for the order of the unusable tracklets behind the last bin, which
+                                        nothing reads. */
     int32_t reserved_;
 } trd_config;
 
