@@ -217,6 +217,26 @@ int trd_set_chamber_dx(trd_handle* h, const float* dx, int32_t n_chambers, void*
 int trd_match(trd_handle* h, const trd_tracks_in* in, const trd_tracks_out* out, int64_t n_tracks,
               void* stream);
 
+/* trd_match for callers that cannot allocate device memory (code under CUDA graph capture, serving loops, harnesses
+ * that forbid cudaMalloc): the same tracking step (as trd_match above), on the track-binned path, with
+ * every scratch buffer (packed track and result records, locality keys, permutation, key histogram) in ONE file-scope
+ * device array of TRD_STATIC_SCRATCH_BYTES (7.5 MiB) that is part of the library's device image: every GPU that loads
+ * the library holds it until the process exits.  The call allocates and frees nothing -- no cudaMalloc, cudaFree,
+ * event or stream creation, no allocating library routine -- and only enqueues a memset and five kernels on `stream`.
+ *   in, out     device arrays as for trd_match (the caller's; same layout, same ownership); results are those of
+ *               trd_match on the same input (the order in which tracks are processed changes no result)
+ *   n_tracks    0 .. TRD_STATIC_MAX_TRACKS; more is refused with TRD_E_ARG and a text in trd_last_error
+ *   index       the tracklets must have been loaded before (trd_load_tracklets allocates; this call does not)
+ * TRD_E_ARG also when the track locality key of this configuration is wider than 16 bits (time-frame association with
+ * more than about 40 interactions): use trd_match there.
+ * The array is shared by every call, handle and host thread of the process on that GPU and keeps the last call's
+ * contents (the library clears the part that must start at zero): calls that overlap on the GPU -- different streams,
+ * or different handles on the same device -- race on it.  Serialise them on one stream or with events. */
+#define TRD_STATIC_MAX_TRACKS 32768
+#define TRD_STATIC_SCRATCH_BYTES 7864320   /* 32768 x (96 + 128 + 4 + 4) + 4 x 65536 */
+int trd_match_static(trd_handle* h, const trd_tracks_in* in, const trd_tracks_out* out, int64_t n_tracks,
+                     void* stream);
+
 /* TRD-only refit of the matched chains (calibration step 3: refits "ignoring the TPC clusters";
  * PAPER.md:9): for every track with at least two attached tracklets the matcher's final state is taken
  * as the starting point, its covariance is reset to diag(refit_var), the Kalman filter runs INWARD over the attached

@@ -20,7 +20,7 @@ TRD_MAX_HYP = 8
 TRD_OK, TRD_E_ARG, TRD_E_CUDA, TRD_E_NOMEM, TRD_E_STATE = 0, -1, -2, -3, -4
 _STATUS = {0: "TRD_OK", -1: "TRD_E_ARG", -2: "TRD_E_CUDA", -3: "TRD_E_NOMEM", -4: "TRD_E_STATE"}
 
-EXPORTS = ("trd_version", "trd_create", "trd_destroy", "trd_load_tracklets", "trd_load_tracklets_tf", "trd_set_chamber_dx", "trd_match", "trd_refit",
+EXPORTS = ("trd_version", "trd_create", "trd_destroy", "trd_load_tracklets", "trd_load_tracklets_tf", "trd_set_chamber_dx", "trd_match", "trd_match_static", "trd_refit",
            "trd_load_tracklets_host", "trd_match_host", "trd_match_host_async", "trd_wait_host", "trd_get_index_info", "trd_copy_index",
            "trd_last_error", "trd_device_bytes", "trd_kernel_launches", "trd_last_match_kernel_ms", "trd_match_kernel_ms")
 
@@ -99,6 +99,7 @@ def lib():
                                             C.c_int64, C.c_void_p]
         l.trd_set_chamber_dx.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]
         l.trd_match.argtypes = [C.c_void_p, C.POINTER(TrdTracksIn), C.POINTER(TrdTracksOut), C.c_int64, C.c_void_p]
+        l.trd_match_static.argtypes = l.trd_match.argtypes
         l.trd_refit.argtypes = [C.c_void_p, C.POINTER(TrdTracksOut), C.POINTER(TrdRefitOut), C.c_int64, C.c_void_p]
         l.trd_match_host.argtypes = l.trd_match.argtypes
         l.trd_match_host_async.argtypes = l.trd_match.argtypes
@@ -249,6 +250,34 @@ def trd_match(h, tracks: dict, out: Optional[dict] = None, n_tracks: Optional[in
         tout.n_matched = _dev_ptr(out["n_matched"], "i32", n)
         tout.n_cand_evals = _dev_ptr(out["n_evals"], "i32", n) if "n_evals" in out else None
     _check(h, lib().trd_match(h, C.byref(tin), C.byref(tout), n, _stream(stream)))
+    return out
+
+
+TRD_STATIC_MAX_TRACKS = 32768          # include/trdmatch.h
+TRD_STATIC_SCRATCH_BYTES = 7864320
+
+
+def trd_match_static(h, tracks: dict, out: dict, n_tracks: Optional[int] = None, stream=None) -> dict:
+    """trd_match without any device allocation: the library's scratch is a static device array, `out` must be given
+    (this wrapper allocates nothing either).  At most TRD_STATIC_MAX_TRACKS tracks per call; calls that overlap on the
+    GPU race on the shared scratch (include/trdmatch.h)."""
+    n = tracks["x"].numel() if n_tracks is None else n_tracks
+    tin, tout = TrdTracksIn(), TrdTracksOut()
+    if n > 0:
+        tin.par[:] = _row_ptrs(tracks["par"], 5, n, "f32")
+        tin.cov[:] = _row_ptrs(tracks["cov"], 15, n, "f32")
+        tin.x = _dev_ptr(tracks["x"], "f32", n)
+        tin.sector = _dev_ptr(tracks["sector"], "i32", n)
+        tin.interaction = _dev_ptr(tracks["interaction"], "i32", n) if "interaction" in tracks else None
+        tout.tracklet_idx[:] = _row_ptrs(out["idx"], TRD_MAX_LAYERS, n, "i32")
+        tout.par[:] = _row_ptrs(out["par"], 5, n, "f32")
+        tout.cov[:] = _row_ptrs(out["cov"], 15, n, "f32")
+        tout.x = _dev_ptr(out["x"], "f32", n)
+        tout.sector = _dev_ptr(out["sector"], "i32", n)
+        tout.chi2 = _dev_ptr(out["chi2"], "f32", n)
+        tout.n_matched = _dev_ptr(out["n_matched"], "i32", n)
+        tout.n_cand_evals = _dev_ptr(out["n_evals"], "i32", n) if "n_evals" in out else None
+    _check(h, lib().trd_match_static(h, C.byref(tin), C.byref(tout), n, _stream(stream)))
     return out
 
 

@@ -277,6 +277,32 @@ int trd_match(trd_handle* h, const trd_tracks_in* in, const trd_tracks_out* out,
     return TRD_OK;
 }
 
+int trd_match_static(trd_handle* h, const trd_tracks_in* in, const trd_tracks_out* out, int64_t n_tracks, void* stream) {
+    if (!h) return TRD_E_ARG;
+    const trd::DeviceGuard on_device(h);
+    if (!in || !out || n_tracks < 0) return fail(h, TRD_E_ARG, "trd_match_static: NULL struct or negative n_tracks");
+    if (n_tracks > TRD_STATIC_MAX_TRACKS)
+        return fail(h, TRD_E_ARG, "trd_match_static: n_tracks = " + std::to_string(n_tracks) + " exceeds TRD_STATIC_MAX_TRACKS = " +
+                                      std::to_string(TRD_STATIC_MAX_TRACKS) + " (the static scratch array holds no more; use trd_match)");
+    if (!h->index_loaded) return fail(h, TRD_E_STATE, "trd_match_static: no tracklets loaded");
+    if (trd::track_key_bits(h) > trd::kCountingBits)
+        return fail(h, TRD_E_ARG, "trd_match_static: the track locality key of this configuration is wider than 16 bits (use trd_match)");
+    if (n_tracks == 0) return TRD_OK;
+    for (int k = 0; k < 5; ++k)
+        if (!in->par[k] || !out->par[k]) return fail(h, TRD_E_ARG, "trd_match_static: NULL par array");
+    for (int k = 0; k < 15; ++k)
+        if (!in->cov[k] || !out->cov[k]) return fail(h, TRD_E_ARG, "trd_match_static: NULL cov array");
+    for (int l = 0; l < TRD_MAX_LAYERS; ++l)
+        if (!out->tracklet_idx[l]) return fail(h, TRD_E_ARG, "trd_match_static: NULL tracklet_idx array");
+    if (!in->x || !in->sector || !out->x || !out->sector || !out->chi2 || !out->n_matched)
+        return fail(h, TRD_E_ARG, "trd_match_static: NULL array");
+    if (h->mp.g.n_ia > 1 && !in->interaction)
+        return fail(h, TRD_E_ARG, "trd_match_static: the index carries interactions but trd_tracks_in.interaction is NULL");
+    const cudaError_t e = trd::launch_match_static(h, *in, *out, n_tracks, (cudaStream_t)stream);
+    if (e != cudaSuccess) return fail_cuda(h, e, "trd_match_static");
+    return TRD_OK;
+}
+
 int trd_get_index_info(const trd_handle* h, trd_index_info* info) {
     if (!h || !info) return TRD_E_ARG;
     if (!h->index_loaded) return TRD_E_STATE;

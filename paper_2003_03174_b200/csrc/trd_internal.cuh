@@ -150,6 +150,9 @@ cudaError_t launch_match(trd_handle* h, const trd_tracks_in& in, const trd_track
                          cudaStream_t stream);
 cudaError_t launch_refit(trd_handle* h, const trd_tracks_out& matched, const trd_refit_out& out, int64_t n,
                          cudaStream_t stream);
+// trd_match_static (match.cu): the binned path with its scratch in a file-scope device array, no allocation of any kind
+cudaError_t launch_match_static(trd_handle* h, const trd_tracks_in& in, const trd_tracks_out& out, int64_t n,
+                                cudaStream_t stream);
 
 // packed track records used when a batch is binned before matching (tracks.cu, match.cu)
 constexpr int kRecIn = 24;    // y z s t c | 15 cov | x | sector bits | 2 pad          (96 bytes)
