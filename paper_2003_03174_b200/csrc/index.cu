@@ -6,12 +6,15 @@
 //       gather_store     sorted store: one float4 (y, z, dy/dx, position) per tracklet
 //   a3  (in gather_store) first sorted position of every bin (plus sentinel), z extent of every row
 //
-// Large loads take a counting sort instead of the radix passes (same result): the key kernel also counts every
-// bin, one inclusive scan turns the counts into first positions, place_tracklets puts every tracklet at the next
-// free position of its bin (atomic cursor = the table itself, which ends as the first-position table), and
-// order_bins restores the caller's order inside every bin (insertion sort by position, one thread per bin) and
-// records the z extents.  A bin longer than kMaxBin sets a device flag: the counting kernels after it return at
-// once and the radix kernels, enqueued behind them and gated on the same flag, do the work -- no host round trip.
+// Large loads take a counting sort instead of the radix passes (same result): the key kernel also counts every bin
+// and keeps the value the count had as the tracklet's rank inside its bin (one byte; the atomics run in the caller's
+// order, block after block, so a bin is filled almost in that order), one inclusive scan turns the counts into first
+// positions, partition_tracklets groups the tracklets by the leading digit of the key so that the placement that follows
+// writes complete lines in L2, place_tracklets puts every tracklet at first(bin) + rank without an atomic, and
+// order_bins restores the caller's order inside every bin where the ranks did not give it (insertion sort by position,
+// one thread per bin) and records the z extents.  A bin longer than kMaxBin sets a device flag: the placement kernels
+// return at once and the one-launch sort of small loads (small_index), enqueued behind them and gated on the same
+// flag, builds the index instead -- no host round trip.  Loads of up to 2^18 tracklets take small_index directly.
 //
 // north_star: "device-side sort and index by chamber and local-y bin ... a radix sort plus
 // per-chamber y-bin offsets"; the 18 x 5 x 6 segmentation is PAPER.md:50.  The key also
@@ -51,24 +54,45 @@ __global__ void __launch_bounds__(256) tracklet_key(const float* __restrict__ y,
                                                     const float* __restrict__ dydx, const int32_t* __restrict__ chamber,
                                                     const int32_t* __restrict__ interaction, uint32_t* __restrict__ key,
                                                     float4* __restrict__ packed, int64_t n, IndexGeom g,
-                                                    uint32_t* __restrict__ digit_tot, int shift) {
+                                                    uint32_t* __restrict__ digit_tot, int shift,
+                                                    uint32_t* __restrict__ count, uint8_t* __restrict__ rank) {
     // digit_tot (counting sort): how many keys carry each leading digit, for the partition that follows
     __shared__ uint32_t cnt[kRadix];
     if (digit_tot) {
         cnt[threadIdx.x] = 0;
         __syncthreads();
     }
+    const int64_t i0 = (int64_t)blockIdx.x * kKeyItems * 256 + threadIdx.x;
+    float yy[kKeyItems], zz[kKeyItems], dd[kKeyItems];
+    int ch[kKeyItems], ia[kKeyItems];
+    uint32_t k[kKeyItems], rk[kKeyItems];
 #pragma unroll
     for (int u = 0; u < kKeyItems; ++u) {
-        const int64_t i = ((int64_t)blockIdx.x * kKeyItems + u) * 256 + threadIdx.x;
-        if (i >= n) break;
-        const float yy = y[i], zz = z[i];
-        const int ch = chamber[i];
-        packed[i] = make_float4(yy, zz, dydx[i], __int_as_float(ch));
-        const int ia = (g.n_ia > 1) ? interaction[i] : 0;      // time-frame association: the interaction leads the key
-        const uint32_t k = key_of(g, yy, zz, ch, ia);
-        key[i] = k;
-        if (digit_tot) atomicAdd(&cnt[(k >> shift) & (kRadix - 1)], 1u);
+        const int64_t i = i0 + u * 256;
+        yy[u] = zz[u] = dd[u] = 0.0f;
+        ch[u] = -1;
+        ia[u] = 0;
+        if (i < n) {
+            yy[u] = __ldcs(y + i); zz[u] = __ldcs(z + i); dd[u] = __ldcs(dydx + i);   // streamed: the count table stays in L2
+            ch[u] = __ldcs(chamber + i);
+            if (g.n_ia > 1) ia[u] = __ldcs(interaction + i);            // time-frame association: the interaction leads the key
+        }
+    }
+#pragma unroll
+    for (int u = 0; u < kKeyItems; ++u) {
+        k[u] = key_of(g, yy[u], zz[u], ch[u], ia[u]);
+        rk[u] = 0u;
+        if (count && i0 + u * 256 < n) rk[u] = atomicAdd(count + k[u] + 1, 1u);   // all in flight before the first is used
+    }
+#pragma unroll
+    for (int u = 0; u < kKeyItems; ++u) {
+        const int64_t i = i0 + u * 256;
+        if (i < n) {
+            __stcs(packed + i, make_float4(yy[u], zz[u], dd[u], __int_as_float(ch[u])));
+            __stcs(key + i, k[u]);
+            if (digit_tot) atomicAdd(&cnt[(k[u] >> shift) & (kRadix - 1)], 1u);
+            if (count) __stcs(rank + i, (uint8_t)min(rk[u], 255u));
+        }
     }
     if (digit_tot) {
         __syncthreads();
@@ -227,23 +251,24 @@ __global__ void __launch_bounds__(kSortThreads, 3) radix_scatter(const uint32_t*
     }
 }
 
-// First step of the counting sort: partition by the leading digit of the key, the tracklet itself travelling along
-// (rec_out gets (y, z, dy/dx, position), dx_out the radial offset of its chamber), every bin counted on the way
-// (count[key + 2]: the inclusive scan leaves first(k) at [k + 1]), so that the placement that follows finds the
-// tracklets of one bucket, and their bins, close together in L2.  The order inside a bucket is free (order_bins
-// restores the caller's order), hence no stable ranking: ranks inside the tile and the tile's place inside the bucket
-// come from atomic counters; the tile is reordered in shared memory so that the global writes are runs per digit.
+// Counting sort of large loads: partition by the leading digit of the key, the tracklet itself travelling along (rec_out
+// gets (y, z, dy/dx, position), dx_out the radial offset of its chamber, rank_out its rank inside its bin), so that the
+// placement that follows finds the tracklets of one bucket, and their bins, close together in L2.  The order inside a
+// bucket is free, hence no stable ranking: ranks inside the tile and the tile's place inside the bucket come from atomic
+// counters; the tile is reordered in shared memory so that the global writes are runs per digit.
 struct Partition {
     const float4* packed;
     float4* rec_out;
     const float* chamber_dx;
     float* dx_out;
     uint32_t* count;
+    const uint8_t* rank_in; // place of the tracklet inside its bin (the value the count had when the key kernel counted it)
+    uint8_t* rank_out;
     int n_chambers;
 };
 constexpr int kPartItems = 8;
 constexpr int kPartTile = 256 * kPartItems;
-constexpr size_t kPartSmem = (size_t)kPartTile * (sizeof(float4) + 2 * sizeof(uint32_t));
+constexpr size_t kPartSmem = (size_t)kPartTile * (sizeof(float4) + 2 * sizeof(uint32_t) + 1);
 
 __global__ void __launch_bounds__(256) partition_tracklets(const uint32_t* __restrict__ key_in, uint32_t* __restrict__ key_out,
                                                            const Partition pl, const uint32_t* __restrict__ digit_tot,
@@ -252,6 +277,7 @@ __global__ void __launch_bounds__(256) partition_tracklets(const uint32_t* __res
     float4* const s_rec = s_dyn;
     uint32_t* const s_key = reinterpret_cast<uint32_t*>(s_rec + kPartTile);
     uint32_t* const s_pos = s_key + kPartTile;
+    uint8_t* const s_rank = reinterpret_cast<uint8_t*>(s_pos + kPartTile);
     __shared__ uint32_t s_cnt[kRadix], s_base[kRadix], s_off[kRadix];
     __shared__ uint32_t warp_sums[32];
     __shared__ uint32_t total;
@@ -259,15 +285,18 @@ __global__ void __launch_bounds__(256) partition_tracklets(const uint32_t* __res
     const uint32_t start = block_exclusive_scan(digit_tot[threadIdx.x], warp_sums, &total);     // syncs
     const int64_t tile_base = (int64_t)blockIdx.x * kPartTile;
     uint32_t k[kPartItems], rank[kPartItems];
+    uint8_t rb[kPartItems];
     float4 r[kPartItems];
 #pragma unroll
     for (int u = 0; u < kPartItems; ++u) {
         const int64_t i = tile_base + u * 256 + threadIdx.x;
         k[u] = 0u;
+        rb[u] = 0;
         r[u] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
         if (i < n) {
             k[u] = key_in[i];
             r[u] = pl.packed[i];
+            rb[u] = pl.rank_in[i];
         }
     }
 #pragma unroll
@@ -288,6 +317,7 @@ __global__ void __launch_bounds__(256) partition_tracklets(const uint32_t* __res
             s_rec[lp] = r[u];
             s_key[lp] = k[u];
             s_pos[lp] = (uint32_t)i;
+            s_rank[lp] = rb[u];
         }
     }
     __syncthreads();
@@ -306,7 +336,7 @@ __global__ void __launch_bounds__(256) partition_tracklets(const uint32_t* __res
                 const int ch = __float_as_int(tl.w);
                 pl.dx_out[dst] = (ch >= 0 && ch < pl.n_chambers) ? __ldg(pl.chamber_dx + ch) : 0.0f;
             }
-            atomicAdd(pl.count + kk + 2, 1u);
+            pl.rank_out[dst] = s_rank[j];
         }
     }
 }
@@ -380,7 +410,7 @@ constexpr int kMaxBin = 32;                         // longest bin order_bins so
 constexpr int kScanItems = 16;
 constexpr int kScanChunk = 256 * kScanItems;        // table entries per block
 
-// sum of every chunk of the count table; flags a bin (entries 2 .. n_bins + 1; the unusable tracklets behind them
+// sum of every chunk of the count table; flags a bin (entries 1 .. n_bins; the unusable tracklets behind them
 // are never read and need no order) longer than kMaxBin
 __global__ void __launch_bounds__(256) count_reduce(const uint32_t* __restrict__ tab, uint32_t* __restrict__ partial, int64_t m,
                                                     int64_t n_bins, int* __restrict__ flag) {
@@ -403,7 +433,7 @@ __global__ void __launch_bounds__(256) count_reduce(const uint32_t* __restrict__
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
             sum += v[u];
-            if (j + u >= 2 && j + u < n_bins + 2) longest = max(longest, v[u]);
+            if (j + u >= 1 && j + u < n_bins + 1) longest = max(longest, v[u]);
         }
     }
     if (longest > (uint32_t)kMaxBin) *flag = 1;
@@ -459,18 +489,21 @@ __global__ void __launch_bounds__(256) count_apply(uint32_t* __restrict__ tab, c
     }
 }
 
-// every tracklet to the next free position of its bin.  tab[k + 1] starts as first(k) and ends as first(k + 1):
-// afterwards tab[b] = first sorted position whose key is >= b, the table the match kernel reads.
-// The input is partitioned by the leading key digit (partition_tracklets): the blocks running at one time work on a
-// few buckets, whose bins and store lines stay in L2 until they are complete.
-__global__ void __launch_bounds__(256) place_tracklets(const uint32_t* __restrict__ key, const float4* __restrict__ rec,
-                                                       const float* __restrict__ rec_dx, uint32_t* __restrict__ tab,
+// every tracklet to its place: tab[k] = first sorted position whose key is >= k (the table the match kernel reads), rank
+// from the key kernel.  The input is partitioned by the leading key digit (partition_tracklets): the blocks running at
+// one time work on a few buckets, whose table entries and store lines stay in L2 until they are complete.
+__global__ void __launch_bounds__(256) place_tracklets(const uint32_t* __restrict__ key, const uint8_t* __restrict__ rank,
+                                                       const float4* __restrict__ rec, const float* __restrict__ rec_dx,
+                                                       const uint32_t* __restrict__ tab, uint32_t* __restrict__ cursor,
                                                        float4* __restrict__ store, float* __restrict__ store_dx, int64_t n,
-                                                       const int* __restrict__ flag) {
+                                                       uint32_t n_bins, const int* __restrict__ flag) {
     if (*flag != 0) return;
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
-    const uint32_t pos = atomicAdd(tab + key[i] + 1, 1u);      // one tracklet per thread: more per thread measured slower
+    const uint32_t k = key[i];
+    // usable tracklets: first position of the bin + the rank taken when the bin was counted (bins are at most kMaxBin long
+    // here); the unusable ones behind the last bin, in any order
+    const uint32_t pos = __ldg(tab + k) + (k < n_bins ? (uint32_t)rank[i] : atomicAdd(cursor, 1u));
     store[pos] = rec[i];
     if (store_dx) store_dx[pos] = rec_dx[i];
 }
@@ -946,7 +979,7 @@ cudaError_t build_index(trd_handle* h, const float* d_y, const float* d_z, const
     // counting sort: when asked for, or for loads large enough that the radix passes cost more than its extra launches
     const bool counting = c.index_sort > 0 || (c.index_sort == 0 && n >= kCountingMin);
     h->sort_kind = counting ? 1 : 0;
-    const size_t n_tab = (size_t)g.n_bins + 3;           // counts live at [key + 2] (see tracklet_key)
+    const size_t n_tab = (size_t)g.n_bins + 3;           // counts live at [key + 1] (tracklet_key, small_index)
     TRD_TRY(reserve(h->bin_first, n_tab * sizeof(int32_t), stream));
     // z extents per row only without association (with it a row holds a couple of tracklets and the table would be large)
     h->use_row_ext = g.n_ia == 1;
@@ -988,10 +1021,14 @@ cudaError_t build_index(trd_handle* h, const float* d_y, const float* d_z, const
     const int* gate = nullptr;
     // the counting sort first partitions by the leading digit of the key
     const int sh = h->key_bits > kRadixBits ? h->key_bits - kRadixBits : 0;
-    if (counting) TRD_TRY(cudaMemsetAsync(h->digit_tot.p, 0, 2 * kRadix * sizeof(uint32_t), stream));   // totals, cursors
+    if (counting) {
+        TRD_TRY(cudaMemsetAsync(h->digit_tot.p, 0, 2 * kRadix * sizeof(uint32_t), stream));   // totals, cursors
+        TRD_TRY(cudaMemsetAsync(h->bin_first.p, 0, n_tab * sizeof(uint32_t), stream));
+    }
     tracklet_key<<<(unsigned)((n + 256 * kKeyItems - 1) / (256 * kKeyItems)), 256, 0, stream>>>(
         d_y, d_z, d_dydx, d_chamber, d_interaction, (uint32_t*)h->key[0].p, (float4*)h->packed.p, n, g,
-        counting ? (uint32_t*)h->digit_tot.p : nullptr, sh);
+        counting ? (uint32_t*)h->digit_tot.p : nullptr, sh, counting ? (uint32_t*)h->bin_first.p : nullptr,
+        counting ? (uint8_t*)h->val[1].p : nullptr);
     h->launches++;
     if (counting) {
         const int n_chunks = (int)((n_tab + kScanChunk - 1) / kScanChunk);
@@ -999,8 +1036,7 @@ cudaError_t build_index(trd_handle* h, const float* d_y, const float* d_z, const
         TRD_TRY(reserve(h->scan_partial, (size_t)n_chunks * sizeof(uint32_t), stream));
         TRD_TRY(reserve(h->part_rec, (size_t)n * sizeof(float4), stream));
         if (has_dx) TRD_TRY(reserve(h->part_dx, (size_t)n * sizeof(float), stream));
-        TRD_TRY(cudaMemsetAsync(h->sort_flag.p, 0, sizeof(int), stream));
-        TRD_TRY(cudaMemsetAsync(h->bin_first.p, 0, n_tab * sizeof(uint32_t), stream));
+        TRD_TRY(cudaMemsetAsync(h->sort_flag.p, 0, 2 * sizeof(int), stream));      // flag, cursor of the unusable tracklets
         uint32_t* tab = (uint32_t*)h->bin_first.p;
         int* flag = (int*)h->sort_flag.p;
         Partition pl;
@@ -1009,6 +1045,8 @@ cudaError_t build_index(trd_handle* h, const float* d_y, const float* d_z, const
         pl.chamber_dx = has_dx ? (const float*)h->chamber_dx.p : nullptr;
         pl.dx_out = has_dx ? (float*)h->part_dx.p : nullptr;
         pl.count = tab;
+        pl.rank_in = (const uint8_t*)h->val[1].p;
+        pl.rank_out = (uint8_t*)h->val[0].p;
         pl.n_chambers = g.n_chambers;
         TRD_TRY(cudaFuncSetAttribute(partition_tracklets, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kPartSmem));
         partition_tracklets<<<(unsigned)((n + kPartTile - 1) / kPartTile), 256, kPartSmem, stream>>>(
@@ -1016,9 +1054,10 @@ cudaError_t build_index(trd_handle* h, const float* d_y, const float* d_z, const
         count_reduce<<<n_chunks, 256, 0, stream>>>(tab, (uint32_t*)h->scan_partial.p, (int64_t)n_tab, (int64_t)g.n_bins, flag);
         count_scan_partials<<<1, 1024, 0, stream>>>((uint32_t*)h->scan_partial.p, n_chunks);
         count_apply<<<n_chunks, 256, 0, stream>>>(tab, (const uint32_t*)h->scan_partial.p, (int64_t)n_tab);
-        place_tracklets<<<(unsigned)((n + 255) / 256), 256, 0, stream>>>((const uint32_t*)h->key[1].p, (const float4*)h->part_rec.p,
-                                                                         has_dx ? (const float*)h->part_dx.p : nullptr, tab, (float4*)h->store.p,
-                                                                         has_dx ? (float*)h->store_dx.p : nullptr, n, flag);
+        place_tracklets<<<(unsigned)((n + 255) / 256), 256, 0, stream>>>((const uint32_t*)h->key[1].p, (const uint8_t*)h->val[0].p,
+                                                                         (const float4*)h->part_rec.p, has_dx ? (const float*)h->part_dx.p : nullptr,
+                                                                         tab, (uint32_t*)h->sort_flag.p + 1, (float4*)h->store.p,
+                                                                         has_dx ? (float*)h->store_dx.p : nullptr, n, g.n_bins, flag);
         order_bins<<<(unsigned)(((int64_t)g.n_bins + 255) / 256), 256, 0, stream>>>(tab, (float4*)h->store.p, has_dx ? (float*)h->store_dx.p : nullptr,
                                                                                     h->use_row_ext ? (uint2*)h->row_ext.p : nullptr,
                                                                                     (int64_t)g.n_bins, g.nb_shift, flag);

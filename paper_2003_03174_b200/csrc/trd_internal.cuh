@@ -105,7 +105,8 @@ struct trd_handle {
     trd::Buffer store;      // float4 per sorted tracklet: y, z, dy/dx, original position (bits)
     trd::Buffer packed;     // float4 per tracklet in the caller's order (gather source)
     trd::Buffer key[2];     // uint32 keys, ping-pong
-    trd::Buffer val[2];     // uint32 original positions, ping-pong
+    trd::Buffer val[2];     // uint32 original positions, ping-pong; counting sort: one rank byte per tracklet, [1] in the
+                            // caller's order, [0] partitioned
     trd::Buffer tile_hist;  // [256][n_tiles] digit counts per tile
     trd::Buffer digit_tot;  // [256]
     trd::Buffer bin_first;  // [n_bins + 1]
