@@ -233,7 +233,7 @@ int trd_match(trd_handle* h, const trd_tracks_in* in, const trd_tracks_out* out,
  * contents (the library clears the part that must start at zero): calls that overlap on the GPU -- different streams,
  * or different handles on the same device -- race on it.  Serialise them on one stream or with events. */
 #define TRD_STATIC_MAX_TRACKS 32768
-#define TRD_STATIC_SCRATCH_BYTES 7864320   /* 32768 x (96 + 128 + 4 + 4) + 4 x 65536 */
+#define TRD_STATIC_SCRATCH_BYTES 7864576   /* 32768 x (96 + 128 + 4 + 4) + 4 x 65536 + 256 */
 int trd_match_static(trd_handle* h, const trd_tracks_in* in, const trd_tracks_out* out, int64_t n_tracks,
                      void* stream);
 

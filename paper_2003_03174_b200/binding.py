@@ -254,7 +254,7 @@ def trd_match(h, tracks: dict, out: Optional[dict] = None, n_tracks: Optional[in
 
 
 TRD_STATIC_MAX_TRACKS = 32768          # include/trdmatch.h
-TRD_STATIC_SCRATCH_BYTES = 7864320
+TRD_STATIC_SCRATCH_BYTES = 7864576
 
 
 def trd_match_static(h, tracks: dict, out: dict, n_tracks: Optional[int] = None, stream=None) -> dict:

@@ -101,21 +101,27 @@ __global__ void __launch_bounds__(kThreads) unpack_kernel(const float* __restric
     if (out.n_cand_evals) out.n_cand_evals[i] = __float_as_int(r[30]);
 }
 
-// counting sort, step 2: exclusive scan of the key histogram in place (one block)
-constexpr int kScanThreads = 1024;
-constexpr int kScanMax = (1 << kCountingBits) / kScanThreads;      // keys per thread at most (64)
-__global__ void __launch_bounds__(kScanThreads) scan_hist(uint32_t* __restrict__ hist, int per4) {
-    // thread t owns the 4 * per4 consecutive keys from t * 4 * per4 (n_keys = 1024 * 4 * per4, a power of two >= 4096);
-    // 16-byte loads, all issued before the first use
-    __shared__ uint32_t warp_sums[32];
+// counting sort, step 2: exclusive scan of the key histogram in place.  One block per tile of 4096 keys (1 to 16 blocks);
+// a block publishes its tile's sum in status[tile] (bit 31 = published; pack_tracks cleared the words together with the
+// histogram) and adds up the sums of the tiles before it, spinning until they are there: those blocks have lower
+// indices and were scheduled first, so they are running.  (One block for the whole table took 15.5 us per call.)
+constexpr int kScanThreads = 256;
+constexpr int kScanPer = 16;                                       // keys per thread
+constexpr int kScanTile = kScanThreads * kScanPer;                 // 4096 = the smallest table (track_key_bits >= 12)
+constexpr int kScanMaxTiles = (1 << kCountingBits) / kScanTile;    // 16 status words
+constexpr uint32_t kPublished = 0x80000000u;
+constexpr int kStatusWords = 64;                                   // 256 bytes in front of the histogram (kTrackHistBytes)
+__global__ void __launch_bounds__(kScanThreads) scan_hist(uint32_t* __restrict__ hist, uint32_t* __restrict__ status) {
+    __shared__ uint32_t warp_sums[kScanThreads / 32];
+    __shared__ uint32_t s_before;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    uint4* mine = reinterpret_cast<uint4*>(hist) + (size_t)threadIdx.x * per4;
-    uint4 c[kScanMax / 4];
+    uint4* mine = reinterpret_cast<uint4*>(hist) + ((size_t)blockIdx.x * kScanThreads + threadIdx.x) * (kScanPer / 4);
+    uint4 c[kScanPer / 4];
 #pragma unroll
-    for (int k = 0; k < kScanMax / 4; ++k) c[k] = (k < per4) ? mine[k] : make_uint4(0u, 0u, 0u, 0u);
+    for (int k = 0; k < kScanPer / 4; ++k) c[k] = mine[k];
     uint32_t sum = 0;
 #pragma unroll
-    for (int k = 0; k < kScanMax / 4; ++k) sum += c[k].x + c[k].y + c[k].z + c[k].w;
+    for (int k = 0; k < kScanPer / 4; ++k) sum += c[k].x + c[k].y + c[k].z + c[k].w;
     uint32_t incl = sum;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
@@ -125,29 +131,40 @@ __global__ void __launch_bounds__(kScanThreads) scan_hist(uint32_t* __restrict__
     if (lane == 31) warp_sums[warp] = incl;
     __syncthreads();
     if (warp == 0) {
-        const uint32_t w = warp_sums[lane];
+        const uint32_t w = lane < kScanThreads / 32 ? warp_sums[lane] : 0u;
         uint32_t wi = w;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
             const uint32_t t = __shfl_up_sync(0xffffffffu, wi, o);
             if (lane >= o) wi += t;
         }
-        warp_sums[lane] = wi - w;
+        if (lane < kScanThreads / 32) warp_sums[lane] = wi - w;
+        const uint32_t total = __shfl_sync(0xffffffffu, wi, 31);
+        volatile uint32_t* st = status;
+        if (lane == 0) st[blockIdx.x] = kPublished | total;        // at most 2^31 - 1 tracks per call
+        uint32_t before = 0;                                       // tiles before this one: at most 15, one lane each
+        if (lane < (int)blockIdx.x) {
+            uint32_t v;
+            do { v = st[lane]; } while (!(v & kPublished));
+            before = v & ~kPublished;
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) before += __shfl_xor_sync(0xffffffffu, before, o);
+        if (lane == 0) s_before = before;
     }
     __syncthreads();
-    uint32_t run = warp_sums[warp] + incl - sum;
+    uint32_t run = s_before + warp_sums[warp] + incl - sum;
 #pragma unroll
-    for (int k = 0; k < kScanMax / 4; ++k) {
-        if (k < per4) {
-            uint4 o;
-            o.x = run; run += c[k].x;
-            o.y = run; run += c[k].y;
-            o.z = run; run += c[k].z;
-            o.w = run; run += c[k].w;
-            mine[k] = o;
-        }
+    for (int k = 0; k < kScanPer / 4; ++k) {
+        uint4 o;
+        o.x = run; run += c[k].x;
+        o.y = run; run += c[k].y;
+        o.z = run; run += c[k].z;
+        o.w = run; run += c[k].w;
+        mine[k] = o;
     }
 }
+static_assert(kScanMaxTiles <= 32 && kScanMaxTiles <= kStatusWords, "one lane per earlier tile");
 
 // counting sort, step 3: every track takes the next free place of its key
 __global__ void __launch_bounds__(256) place_tracks(const uint32_t* __restrict__ key, uint32_t* __restrict__ next,
@@ -169,10 +186,11 @@ cudaError_t pack_tracks(trd_handle* h, const trd_tracks_in& in, int64_t n, float
     const int bits = track_key_bits(h);
     if (bits > kCountingBits) hist = nullptr;
     if (hist) {
-        cudaError_t e = cudaMemsetAsync(hist, 0, sizeof(uint32_t) << bits, stream);
+        // the status words of scan_hist and, behind them, the histogram
+        cudaError_t e = cudaMemsetAsync(hist, 0, kStatusWords * sizeof(uint32_t) + (sizeof(uint32_t) << bits), stream);
         if (e != cudaSuccess) return e;
     }
-    pack_kernel<<<grid, kThreads, 0, stream>>>(in, n, rec, key, g, x_mid, edge_mid, g.nz, hist);
+    pack_kernel<<<grid, kThreads, 0, stream>>>(in, n, rec, key, g, x_mid, edge_mid, g.nz, hist ? hist + kStatusWords : nullptr);
     h->launches++;
     *key_bits = bits;
     return cudaGetLastError();
@@ -190,8 +208,8 @@ int track_key_bits(const trd_handle* h) {
 // counting sort of the tracks by the key histogram pack_tracks filled: perm[place] = track
 cudaError_t place_tracks_by_key(trd_handle* h, const uint32_t* key, uint32_t* hist, uint32_t* perm, int key_bits, int64_t n,
                                 cudaStream_t stream) {
-    scan_hist<<<1, kScanThreads, 0, stream>>>(hist, (1 << key_bits) / (4 * kScanThreads));
-    place_tracks<<<(unsigned)((n + 255) / 256), 256, 0, stream>>>(key, hist, perm, n);
+    scan_hist<<<(1 << key_bits) / kScanTile, kScanThreads, 0, stream>>>(hist + kStatusWords, hist);
+    place_tracks<<<(unsigned)((n + 255) / 256), 256, 0, stream>>>(key, hist + kStatusWords, perm, n);
     h->launches += 2;
     return cudaGetLastError();
 }

@@ -167,6 +167,8 @@ cudaError_t radix_sort_pairs(uint32_t* key0, uint32_t* key1, uint32_t* val0, uin
 cudaError_t export_sorted_index(trd_handle* h, cudaStream_t stream);
 // tracks.cu: SoA -> packed records + locality key; packed results -> SoA
 constexpr int kCountingBits = 16;     // track keys up to this many bits are counting-sorted (tracks.cu)
+// 256 bytes of status words of the scan (tracks.cu scan_hist) + the key histogram of that sort
+constexpr size_t kTrackHistBytes = (sizeof(uint32_t) << kCountingBits) + 256;
 int track_key_bits(const trd_handle* h);
 cudaError_t pack_tracks(trd_handle* h, const trd_tracks_in& in, int64_t n, float* rec, uint32_t* key, int* key_bits,
                         uint32_t* hist, cudaStream_t stream);
