@@ -56,8 +56,12 @@ cudaError_t load_host(trd_handle* h, const float* y, const float* z, const float
     if (h->tl_pending) TRD_TRY(cudaStreamWaitEvent(h->s_in, h->ev_tl_used, 0));
     char* base = (char*)h->stage_tl.p;
     const void* src[4] = {y, z, dydx, chamber};
-    for (int k = 0; k < 4 && n > 0; ++k)
-        TRD_TRY(cudaMemcpyAsync(base + k * bytes, src[k], bytes, cudaMemcpyHostToDevice, h->s_in));
+    for (int k = 0; k < 4 && n > 0;) {
+        int m = 1;
+        while (k + m < 4 && (const char*)src[k + m] == (const char*)src[k] + (size_t)m * bytes) ++m;
+        TRD_TRY(cudaMemcpyAsync(base + k * bytes, src[k], (size_t)m * bytes, cudaMemcpyHostToDevice, h->s_in));
+        k += m;
+    }
     TRD_TRY(cudaEventRecord(h->ev_tl_in, h->s_in));
     TRD_TRY(cudaStreamWaitEvent(st, h->ev_tl_in, 0));
     TRD_TRY(build_index(h, (const float*)base, (const float*)(base + bytes), (const float*)(base + 2 * bytes),
@@ -97,14 +101,26 @@ cudaError_t match_host_async(trd_handle* h, const trd_tracks_in& in, const trd_t
     dst[b] = out.n_matched; dout.n_matched = (int32_t*)(bo + b * bytes); ++b;
     dst[b] = out.n_cand_evals; dout.n_cand_evals = out.n_cand_evals ? (int32_t*)(bo + b * bytes) : nullptr; ++b;
     // copy in (s_in) -> kernels (caller's stream) -> copy out (s_out)
-    for (int j = 0; j < kInArrays; ++j) TRD_TRY(cudaMemcpyAsync(bi + j * bytes, src[j], bytes, cudaMemcpyHostToDevice, h->s_in));
+    // rows that follow each other in the caller's memory (the rows of one (5, n) or (15, n) array) go as one copy
+    for (int j = 0; j < kInArrays;) {
+        int m = 1;
+        while (j + m < kInArrays && (const char*)src[j + m] == (const char*)src[j] + (size_t)m * bytes) ++m;
+        TRD_TRY(cudaMemcpyAsync(bi + j * bytes, src[j], (size_t)m * bytes, cudaMemcpyHostToDevice, h->s_in));
+        j += m;
+    }
     TRD_TRY(cudaEventRecord(h->ev_in[k], h->s_in));
     TRD_TRY(cudaStreamWaitEvent(st, h->ev_in[k], 0));
     TRD_TRY(launch_match(h, din, dout, n, st));
     TRD_TRY(cudaEventRecord(h->ev_done[k], st));
     TRD_TRY(cudaStreamWaitEvent(h->s_out, h->ev_done[k], 0));
-    for (int j = 0; j < kOutArrays; ++j)
-        if (dst[j]) TRD_TRY(cudaMemcpyAsync(dst[j], bo + j * bytes, bytes, cudaMemcpyDeviceToHost, h->s_out));
+    for (int j = 0; j < kOutArrays;) {
+        int m = 1;
+        if (dst[j]) {
+            while (j + m < kOutArrays && dst[j + m] && (char*)dst[j + m] == (char*)dst[j] + (size_t)m * bytes) ++m;
+            TRD_TRY(cudaMemcpyAsync(dst[j], bo + j * bytes, (size_t)m * bytes, cudaMemcpyDeviceToHost, h->s_out));
+        }
+        j += m;
+    }
     TRD_TRY(cudaEventRecord(h->ev_out[k], h->s_out));
     h->slot_busy[k] = true;
     return cudaSuccess;
