@@ -324,6 +324,55 @@ def test_pipelined_host_entry_points(B):
         B.trd_destroy(h)
 
 
+def test_host_rows_need_not_be_adjacent(B):
+    """The host entry points send rows that follow each other in the caller's memory as one copy (host_api.cu); rows of
+    trd_tracks_in / trd_tracks_out are independent pointers, though: here every row is an allocation of its own, except
+    a few that are made adjacent on purpose (cov rows 3-6 and idx rows 1-2), in an order that does not ascend."""
+    import ctypes as C
+    spec = W.CONFIGS["central8"]; d = W.generate(spec); cfg = W.matcher_config(spec)
+    want = run_gpu(B, cfg, d)
+    n = d["x"].shape[0]
+    keep = []
+
+    def own(a):
+        keep.append(np.ascontiguousarray(a).copy())
+        return keep[-1]
+
+    def ptr(a):
+        return a.ctypes.data
+
+    tin, tout = B.TrdTracksIn(), B.TrdTracksOut()
+    par_rows = [own(d["par"][k]) for k in (4, 2, 0, 3, 1)]                        # allocated in another order
+    tin.par[:] = [ptr(par_rows[(4, 2, 0, 3, 1).index(k)]) for k in range(5)]
+    block = own(d["cov"][3:7])                                                     # four adjacent rows
+    cov_rows = {k: own(d["cov"][k]) for k in range(15) if not 3 <= k < 7}
+    tin.cov[:] = [ptr(block) + 4 * n * (k - 3) if 3 <= k < 7 else ptr(cov_rows[k]) for k in range(15)]
+    x, sector = own(d["x"]), own(d["sector"])
+    tin.x, tin.sector = ptr(x), ptr(sector)
+    o_idx_pair = np.empty((2, n), np.int32)
+    o_idx = {l: np.empty(n, np.int32) for l in (0, 3, 4, 5)}
+    tout.tracklet_idx[:] = [ptr(o_idx_pair) + 4 * n * (l - 1) if l in (1, 2) else ptr(o_idx[l]) for l in range(6)]
+    o_par = [np.empty(n, np.float32) for _ in range(5)][::-1]
+    o_cov = [np.empty(n, np.float32) for _ in range(15)]
+    tout.par[:] = [ptr(a) for a in o_par]
+    tout.cov[:] = [ptr(a) for a in o_cov]
+    o = {k: np.empty(n, t) for k, t in (("x", np.float32), ("sector", np.int32), ("chi2", np.float32),
+                                         ("n_matched", np.int32), ("n_evals", np.int32))}
+    tout.x, tout.sector, tout.chi2, tout.n_matched, tout.n_cand_evals = (ptr(o[k]) for k in ("x", "sector", "chi2", "n_matched", "n_evals"))
+    h = B.trd_create(cfg)
+    try:
+        B.trd_load_tracklets_host(h, d["tl_y"], d["tl_z"], d["tl_dydx"], d["tl_chamber"])
+        assert B.lib().trd_match_host(h, C.byref(tin), C.byref(tout), n, None) == B.TRD_OK
+    finally:
+        B.trd_destroy(h)
+    got_idx = np.stack([o_idx_pair[l - 1] if l in (1, 2) else o_idx[l] for l in range(6)])
+    np.testing.assert_array_equal(got_idx, want["idx"])
+    np.testing.assert_array_equal(np.stack(o_par), want["par"])
+    np.testing.assert_array_equal(np.stack(o_cov), want["cov"])
+    for k in o:
+        np.testing.assert_array_equal(o[k], want[k])
+
+
 @pytest.mark.parametrize("name,n_hyp", [("central", 1), ("central8", 8), ("pileup", 4)])
 def test_resolution_model_and_pad_tilt(B, name, n_hyp):
     """sigma_y(sin phi), sigma_dydx(sin phi) and the +-2 degree pad tilt
