@@ -262,6 +262,22 @@ def test_track_binning_does_not_change_results(B, name):
     check_parity(on, want, cfg, d)
 
 
+@pytest.mark.parametrize("n_ia,key_bits", [(2, 12), (7, 14), (40, 16), (64, 17)])
+def test_track_sort_over_every_key_width(B, n_ia, key_bits):
+    """The track key (interaction, sector, z row) of the binned path is counting-sorted up to 16 bits -- its histogram
+    scanned by 1 to 16 blocks that look back over the tile sums before them (tracks.cu scan_hist) -- and radix-sorted
+    above: one block (12 bits), four, sixteen, and the radix path, each bit-identical to the unbinned kernel, two
+    batches in a row through the same scratch."""
+    spec = dataclasses.replace(W.CONFIGS["pileup"], n_interactions=n_ia)
+    d = W.generate(spec); cfg = W.matcher_config(spec)
+    n_keys = n_ia * cfg["n_sectors"] * 2 * (int(np.ceil(cfg["z_max"] / cfg["pad_length"])) + 1)     # index.cu: z rows
+    assert max(12, int(np.ceil(np.log2(n_keys)))) == key_bits
+    off = run_gpu(B, dict(cfg, track_binning=-1), d)
+    on = run_gpu(B, dict(cfg, track_binning=1), d, batch=13001)
+    for k in ("idx", "par", "cov", "x", "sector", "chi2", "n_matched", "n_evals"):
+        np.testing.assert_array_equal(on[k], off[k], err_msg=k)
+
+
 @pytest.mark.parametrize("name", ["central8", "pileup"])
 def test_zero_penalty_scores_of_zero(B, name):
     """chi2_penalty = 0: the skip-children carry score 0, whose child keys (score bits << 32 | parent | position) are
