@@ -125,7 +125,9 @@ def load_bytes_algorithmic(info: dict, n_tl: int) -> float:
 def load_bytes_model(info: dict, n_tl: int) -> float:
     """What THIS implementation moves with the sort it used: not the roofline's numerator."""
     if info["sort_kind"] == 1:
-        return n_tl * 128.0 + 20.0 * info["n_bins"]
+        # key kernel 16 + 21, partition 21 + 21, placement 21 + 16, order 16 per tracklet; table: cleared, scanned (read,
+        # read + write), read by the placement and by order_bins
+        return n_tl * 132.0 + 24.0 * info["n_bins"]
     return n_tl * (76.0 + 20.0 * info["n_passes"])
 
 
