@@ -585,7 +585,8 @@ def test_random_configurations(B):
 
 @pytest.mark.parametrize("name,extra", [("central", {}), ("pileup", dict(res_model=1, chamber_dx_sigma=0.3)), ("central8", {}),
                                         ("pileup", MATERIAL), ("central", dict(MATERIAL, res_model=1, chamber_dx_sigma=0.3, efficiency=0.6)),
-                                        ("central", FIELD), ("pileup", dict(MATERIAL, **FIELD))])
+                                        ("central", FIELD), ("pileup", dict(MATERIAL, **FIELD)),
+                                        ("timeframe", dict(n_tracks=200000, n_noise=800000, batch=None))])   # config 5's density, a tenth of it
 def test_refit_parity(B, name, extra):
     """SURVEY.md 8(f) NEXT#4 (PAPER.md:33 step 3): the CUDA refit against the oracle's refit, both fed the SAME matched
     chains (the oracle's, cast to float32), under the north_star criteria (parameter floor 5e-5, see below)."""
