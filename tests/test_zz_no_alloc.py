@@ -114,6 +114,31 @@ def test_two_handles_share_the_array_when_serialised(B):
         B.trd_destroy(h1); B.trd_destroy(h4)
 
 
+def test_extended_model_through_the_static_entry_point(B):
+    """The extended instantiation of the kernel (sin(phi)-dependent resolutions and pad tilt, displaced chambers,
+    time-frame association with its interaction ids) behind trd_match_static, twice in a row."""
+    import dataclasses
+    import torch
+    spec = dataclasses.replace(W.CONFIGS["pileup"], res_model=1, chamber_dx_sigma=0.3, n_interactions=5)
+    d = W.generate(spec); cfg = W.matcher_config(spec)
+    dev = B.to_device(d); n = d["x"].shape[0]
+    tracks = dict(part_of(dev, 0, n), interaction=dev["interaction"])
+    h = B.trd_create(cfg)
+    try:
+        B.trd_set_chamber_dx(h, np.ascontiguousarray(d["chamber_dx"], np.float32))
+        B.trd_load_tracklets_tf(h, dev["tl_y"], dev["tl_z"], dev["tl_dydx"], dev["tl_chamber"], dev["tl_interaction"],
+                                d["n_interactions"])
+        want = B.to_numpy(B.trd_match(h, tracks))
+        o1, o2 = B.alloc_tracks_out(n), B.alloc_tracks_out(n)
+        B.trd_match_static(h, tracks, o1)
+        B.trd_match_static(h, tracks, o2)
+        torch.cuda.synchronize()
+        same(B.to_numpy(o1), want); same(B.to_numpy(o2), want)
+        assert int((want["n_matched"] >= 2).sum()) > 0.8 * n
+    finally:
+        B.trd_destroy(h)
+
+
 def test_sizes_beyond_the_maximum_are_refused(B):
     import torch
     spec = W.CONFIGS["tiny"]; d = W.generate(spec); cfg = W.matcher_config(spec)
