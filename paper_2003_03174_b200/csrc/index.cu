@@ -892,9 +892,9 @@ static cudaError_t launch_small_index(trd_handle* h, const float* d_y, const flo
                                       cudaStream_t stream) {
     const IndexGeom& g = h->mp.g;
     const bool has_dx = h->mp.dx_max > 0.0f;
-    TRD_TRY(reserve(h->store, (size_t)n * sizeof(float4), stream));
+    TRD_TRY(reserve(h->store, ((size_t)n + kStorePad) * sizeof(float4), stream));
     TRD_TRY(reserve(h->packed, (size_t)n * sizeof(float4), stream));
-    if (has_dx) TRD_TRY(reserve(h->store_dx, (size_t)n * sizeof(float), stream));
+    if (has_dx) TRD_TRY(reserve(h->store_dx, ((size_t)n + kStorePad) * sizeof(float), stream));
     for (int sd = 0; sd < 2; ++sd) {                                  // [0]: keys in caller order / list of long bins;
         TRD_TRY(reserve(h->key[sd], (size_t)n * sizeof(uint32_t), stream));   // [1]: trd_copy_index exports into these
         TRD_TRY(reserve(h->val[sd], (size_t)n * sizeof(uint32_t), stream));
@@ -1007,10 +1007,10 @@ cudaError_t build_index(trd_handle* h, const float* d_y, const float* d_z, const
         TRD_TRY(cudaMemset2DAsync((char*)h->row_ext.p + sizeof(uint32_t), sizeof(uint2), 0x00, sizeof(uint32_t), n_rows, stream));
     }
     const int n_tiles = (int)((n + kTile - 1) / kTile);
-    TRD_TRY(reserve(h->store, (size_t)n * sizeof(float4), stream));
+    TRD_TRY(reserve(h->store, ((size_t)n + kStorePad) * sizeof(float4), stream));
     TRD_TRY(reserve(h->packed, (size_t)n * sizeof(float4), stream));
     const bool has_dx = h->mp.dx_max > 0.0f;
-    if (has_dx) TRD_TRY(reserve(h->store_dx, (size_t)n * sizeof(float), stream));
+    if (has_dx) TRD_TRY(reserve(h->store_dx, ((size_t)n + kStorePad) * sizeof(float), stream));
     for (int s = 0; s < 2; ++s) {
         TRD_TRY(reserve(h->key[s], (size_t)n * sizeof(uint32_t), stream));
         TRD_TRY(reserve(h->val[s], (size_t)n * sizeof(uint32_t), stream));

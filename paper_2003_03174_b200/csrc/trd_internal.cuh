@@ -156,6 +156,10 @@ cudaError_t launch_match_static(trd_handle* h, const trd_tracks_in& in, const tr
                                 cudaStream_t stream);
 
 // packed track records used when a batch is binned before matching (tracks.cu, match.cu)
+// the match kernel reads the sorted store four tracklets at a time without looking at the end of the run (what lies behind
+// it is masked out afterwards): the store and its companion arrays are allocated this many entries longer
+constexpr int kStorePad = 4;
+
 constexpr int kRecIn = 24;    // y z s t c | 15 cov | x | sector bits | 2 pad          (96 bytes)
 constexpr int kRecOut = 32;   // 6 idx | 5 par | 15 cov | x sector chi2 n_matched n_evals | pad   (128 bytes)
 
