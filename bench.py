@@ -447,10 +447,10 @@ def run_sweep(args):
         outs = [B.alloc_tracks_out(hi - lo, torch.device("cuda", 0)) for lo, hi in bounds]
         h = B.trd_create(cfg)
 
-        def step():
-            B.trd_load_tracklets(h, dev["tl_y"], dev["tl_z"], dev["tl_dydx"], dev["tl_chamber"], stream=stream)
+        def step(s=stream):
+            B.trd_load_tracklets(h, dev["tl_y"], dev["tl_z"], dev["tl_dydx"], dev["tl_chamber"], stream=s)
             for t, o in zip(tracks, outs):
-                B.trd_match(h, t, o, stream=stream)
+                B.trd_match(h, t, o, stream=s)
 
         steps = args.steps if name == "timeframe" else max(args.steps, 50)
         for _ in range(5):
@@ -462,6 +462,22 @@ def run_sweep(args):
             step()
         e1.record(stream); torch.cuda.synchronize()
         gpu_ms = e0.elapsed_time(e1) / steps
+        # the same step captured once in a CUDA graph and replayed (after the warm-up the library allocates nothing, so its
+        # calls can be captured): what a caller who processes event after event with fixed buffers would do
+        side = torch.cuda.Stream()
+        with torch.cuda.stream(side):
+            step(side)
+        torch.cuda.synchronize()
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=side):
+            step(side)
+        graph.replay(); torch.cuda.synchronize()
+        e0.record(stream)
+        for _ in range(steps):
+            graph.replay()
+        e1.record(stream); torch.cuda.synchronize()
+        graph_ms = e0.elapsed_time(e1) / steps
+        del graph
         B.trd_destroy(h)
         n_all = min(ORACLE_SAMPLE_TRACKS, n); n_1t = min(ORACLE_SAMPLE_TRACKS_1T, n)
         ra = O.match(cfg, data, lo=0, hi=n_all, n_threads=cores)
@@ -470,18 +486,19 @@ def run_sweep(args):
         cpu_1t_ms = 1e3 * (r1["seconds"]["index"] + r1["seconds"]["match"] * n / n_1t)
         row = dict(sweep=name, n_tracks=n, n_tracklets=n_tl, n_hyp=spec.n_hyp, n_sigma_road=spec.n_sigma_road,
                    gpu_ms_per_step=gpu_ms, gpu_tracks_per_s=n / (gpu_ms * 1e-3), gpu_steps=steps,
+                   gpu_graph_replay_ms_per_step=graph_ms,
                    oracle_cores=cores, oracle_all_cores_ms=cpu_all_ms, oracle_1_thread_ms=cpu_1t_ms,
                    oracle_sample_tracks=[n_all, n_1t], unit="ms per step (load + match of the whole config)")
         rows.append(row)
         print(json.dumps(row), flush=True)
         del dev, tracks, outs
         torch.cuda.empty_cache()
-    print("\n| config | tracks | tracklets | nHyp | oracle, 1 thread | oracle, %d threads | GPU (B200) | GPU tracks/s |" % rows[0]["oracle_cores"])
-    print("|---|---|---|---|---|---|---|---|")
+    print("\n| config | tracks | tracklets | nHyp | oracle, 1 thread | oracle, %d threads | GPU (B200) | GPU, step replayed as a CUDA graph | GPU tracks/s |" % rows[0]["oracle_cores"])
+    print("|---|---|---|---|---|---|---|---|---|")
     for r in rows:
-        print("| %s | %d | %d | %d | %.1f ms | %.1f ms | %.3f ms | %.3g |" % (
+        print("| %s | %d | %d | %d | %.1f ms | %.1f ms | %.3f ms | %.3f ms | %.3g |" % (
             r["sweep"], r["n_tracks"], r["n_tracklets"], r["n_hyp"], r["oracle_1_thread_ms"], r["oracle_all_cores_ms"],
-            r["gpu_ms_per_step"], r["gpu_tracks_per_s"]))
+            r["gpu_ms_per_step"], r["gpu_graph_replay_ms_per_step"], r["gpu_tracks_per_s"]))
 
 
 def main():

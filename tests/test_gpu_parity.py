@@ -340,6 +340,43 @@ def test_pipelined_host_entry_points(B):
         B.trd_destroy(h)
 
 
+@pytest.mark.parametrize("name,binning", [("central8", -1), ("pileup", 1)])
+def test_load_and_match_can_be_captured_in_a_cuda_graph(B, name, binning):
+    """After one warm-up pass the device entry points allocate nothing (buffers only grow), create no stream and never
+    synchronise: trd_load_tracklets + trd_match can be captured in a CUDA graph and replayed; the replay writes the same
+    results (unbinned and binned path)."""
+    import torch
+    spec = W.CONFIGS[name]; d = W.generate(spec); cfg = dict(W.matcher_config(spec), track_binning=binning)
+    want = run_gpu(B, cfg, d)
+    dev = B.to_device(d); n = d["x"].shape[0]
+    h = B.trd_create(cfg)
+    try:
+        out = B.alloc_tracks_out(n)
+        side = torch.cuda.Stream()
+
+        def step():
+            B.trd_load_tracklets(h, dev["tl_y"], dev["tl_z"], dev["tl_dydx"], dev["tl_chamber"], stream=side)
+            B.trd_match(h, dev, out, stream=side)
+
+        with torch.cuda.stream(side):
+            step()                                           # warm-up: every buffer has its size
+        torch.cuda.synchronize()
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=side):
+            step()
+        for k in out:
+            out[k].fill_(-7)
+        for _ in range(2):
+            graph.replay()
+        torch.cuda.synchronize()
+        got = B.to_numpy(out)
+        for k in ("idx", "par", "cov", "x", "sector", "chi2", "n_matched", "n_evals"):
+            np.testing.assert_array_equal(got[k], want[k], err_msg=k)
+        del graph
+    finally:
+        B.trd_destroy(h)
+
+
 def test_host_rows_need_not_be_adjacent(B):
     """The host entry points send rows that follow each other in the caller's memory as one copy (host_api.cu); rows of
     trd_tracks_in / trd_tracks_out are independent pointers, though: here every row is an allocation of its own, except
