@@ -213,7 +213,10 @@ int trd_set_chamber_dx(trd_handle* h, const float* dx, int32_t n_chambers, void*
  * and Fig. 2: every track is extrapolated to each TRD layer (L52, L64), the tracklets inside the search
  * road derived from its covariance are its candidates (L52), those whose inclination is more than 4 sigma off are
  * excluded (L60), chi2 is computed from y and z only (L52), the best n_hyp hypotheses per layer are kept (L60) and
- * updated with a Kalman filter (L9, L40); tracks are independent (L86). */
+ * updated with a Kalman filter (L9, L40); tracks are independent (L86).
+ * Device memory: the handle's buffers only grow.  The first call of a size allocates (cudaMalloc, which synchronises the
+ * device); calls of the same or a smaller size allocate nothing, only enqueue work on `stream`, and can be captured in a
+ * CUDA graph together with trd_load_tracklets (the time read by trd_last_match_kernel_ms is then that of the capture). */
 int trd_match(trd_handle* h, const trd_tracks_in* in, const trd_tracks_out* out, int64_t n_tracks,
               void* stream);
 
