@@ -216,7 +216,8 @@ int trd_set_chamber_dx(trd_handle* h, const float* dx, int32_t n_chambers, void*
  * updated with a Kalman filter (L9, L40); tracks are independent (L86).
  * Device memory: the handle's buffers only grow.  The first call of a size allocates (cudaMalloc, which synchronises the
  * device); calls of the same or a smaller size allocate nothing, only enqueue work on `stream`, and can be captured in a
- * CUDA graph together with trd_load_tracklets (the time read by trd_last_match_kernel_ms is then that of the capture). */
+ * CUDA graph together with trd_load_tracklets (trd_last_match_kernel_ms then reads the events of the captured call as the
+ * last replay recorded them). */
 int trd_match(trd_handle* h, const trd_tracks_in* in, const trd_tracks_out* out, int64_t n_tracks,
               void* stream);
 
